@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the batched harmonic sum (arXiv 1812.02647 eqs. 1-4) on B200, one JSON line.
+
+A "step" is one pass of the whole hot path over one batch of synthetic spectra: hs_execute of each of the four
+variants (standard, Max, freq-bin, Greedy) at Hmax = 32 in the workload's output mode.  The default workload is
+BASELINE.json configs[2] (4096 spectra x 2^18 bins, Exp(1)-1 noise + 1 % injected combs, reduced output), the
+configuration the metric is quoted on.  `value` = bins/s, one bin = one output bin of one variant, i.e.
+variants x batch x nbins / step time, inputs resident in HBM; `e2e` = the same through hs_execute_host with pinned
+host buffers (host<->device copies inside the timed region).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload config2|config1|config3]
+                    [--batch B] [--variants standard,max,freqbin,greedy] [--algo auto|direct|tiled] [--no-e2e]
+
+N > 1: launched under torchrun, one rank per GPU, every rank runs the same batch shape on its own seeded data
+(weak scaling, spectra are independent: no data-path collective); time = max over ranks.
+`--impl reference` times the CPU oracle (oracle/hs_oracle.c) on a bounded sample of the same workload on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import concurrent.futures
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+VARIANTS = ["standard", "max", "freqbin", "greedy"]
+WORKLOADS = {
+    # name: (batch, nbins, out_mode, description)
+    "config2": (4096, 1 << 18, "reduced", "configs[2]: 4096 x 2^18 Exp(1)-1 noise, 1% combs, reduced output"),
+    "config1": (256, 1 << 18, "both", "configs[1] shape: 256 x 2^18, full and reduced output (Exp(1)-1 stand-in noise)"),
+    "config3": (8, 1 << 23, "full", "configs[3]: 8 x 2^23 Exp(1)-1 noise, one comb each, full output"),
+}
+BYTES_PER_BIN = {"reduced": 4 + 5, "full": 4 + 4 * 6, "both": 4 + 4 * 6 + 5}   # SURVEY.md section 8(d), Hmax = 32
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS))
+    ap.add_argument("--batch", type=int, default=0, help="override the batch (non-headline; recorded in config)")
+    ap.add_argument("--variants", default=",".join(VARIANTS))
+    ap.add_argument("--algo", default="auto", choices=["auto", "direct", "tiled"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
+    return ap.parse_args()
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(variant, workload, algo):
+    """DRAM bytes per launch from the committed ncu capture (profiles/ncu_traffic.json), or None."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json")))[f"{workload}/{variant}/{algo}"]
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [t.strip() for t in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                smax.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v == "Active":
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_rate(x_rows, variants, seconds, threads):
+    """Oracle throughput (bins/s, one bin = one output bin of one variant) on whole spectra of x_rows [R][N],
+    spectra-parallel over `threads` host threads (the paper's CPU strategy; ctypes releases the GIL)."""
+    import oracle
+    oracle.build()
+    R, N = x_rows.shape
+    jobs = [(r, v) for r in range(R) for v in variants]
+    t0 = time.perf_counter()
+    done = 0
+
+    def work(job):
+        r, v = job
+        oracle.harmonic_sum(x_rows[r], 32, v, want_sums=False, want_reduced=True)
+        return N
+
+    with concurrent.futures.ThreadPoolExecutor(max_workers=threads) as ex:
+        futs = []
+        for job in jobs:
+            futs.append(ex.submit(work, job))
+        for f in futs:
+            done += f.result()
+            if time.perf_counter() - t0 > seconds * 4:
+                break
+    dt = time.perf_counter() - t0
+    return done / dt, dt, done
+
+
+def cpu_sample_rows(seconds, threads, nbins, variants):
+    # ~0.7 s of single-thread work per 2^18-bin spectrum for the four variants together
+    per_spectrum = 0.7 * (nbins / float(1 << 18)) * len(variants) / 4.0
+    return max(1, min(64, int(seconds * threads / per_spectrum)))
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores, on a bounded sample of the workload per step."""
+    import numpy as np
+    import workloads as W
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    batch, nbins, out_mode, desc = WORKLOADS[args.workload]
+    variants = args.variants.split(",")
+    threads = os.cpu_count() or 1
+    total_steps = max(1, args.steps + args.warmup)
+    rows = cpu_sample_rows(max(2.0, 120.0 / total_steps), threads, nbins, variants)
+    cfg = {"config2": 2, "config1": 2, "config3": 3}[args.workload]
+    x, _ = W.comb_batch_numpy(cfg, list(range(rows)), nbins, 0.01 if cfg == 2 else 1.0,
+                              50.0 if cfg == 2 else 1000.0, 5000.0 if cfg == 2 else 100000.0, 0.10 if cfg == 2 else 0.03)
+    for _ in range(args.warmup):
+        oracle_rate(x[:max(1, rows // 4)], variants, 1e9, threads)
+    t0 = time.perf_counter()
+    bins = 0
+    for _ in range(args.steps):
+        _, _, done = oracle_rate(x, variants, 1e9, threads)
+        bins += done
+    dt = time.perf_counter() - t0
+    value = bins / dt
+    sample = f"{rows} whole spectra of {nbins} bins x {len(variants)} variants per step (of {batch} in the workload)"
+    line = {"impl": "reference", "metric": "harmonic_sum_bins_per_s", "value": value, "unit": "bins/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": desc, "batch": batch, "nbins": nbins, "Hmax": 32, "out_mode": out_mode,
+                       "variants": variants, "note": "CPU oracle on a bounded sample per step"},
+            "cpu_baseline": {"value": value, "unit": "bins/s", "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "bins/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import workloads as W
+    from paper_1812_02647_b200 import binding as hs
+    from paper_1812_02647_b200.shard import max_over_ranks_ms, sum_over_ranks
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+
+    batch, nbins, out_mode, desc = WORKLOADS[args.workload]
+    if args.batch:
+        batch = args.batch
+    variants = args.variants.split(",")
+    L = 6
+
+    # ---- inputs, resident in HBM (seeded; every rank draws its own batch: weak scaling) -----------------------------
+    cfg = {"config2": 2, "config1": 2, "config3": 3}[args.workload]
+    x = W.exp_noise_torch(batch, nbins, cfg + 100 * rank, dev)
+    if args.workload == "config3":
+        W.inject_combs_torch(x, 3, 1.0, 1000.0, 100000.0, 0.03)
+    else:
+        W.inject_combs_torch(x, 2, 0.01, 50.0, 5000.0, 0.10)
+    sums = torch.empty((batch, L, nbins), dtype=torch.float32, device=dev) if out_mode in ("full", "both") else None
+    vmax = torch.empty((batch, nbins), dtype=torch.float32, device=dev) if out_mode in ("reduced", "both") else None
+    amax = torch.empty((batch, nbins), dtype=torch.uint8, device=dev) if out_mode in ("reduced", "both") else None
+    plans = {}
+    for v in variants:
+        p = hs.hs_plan_create(nbins, batch, 32, v, out_mode)
+        p.set_algo(args.algo)
+        p.ensure_workspace(dev)
+        plans[v] = p
+    algo_names = {hs.HS_ALGO_DIRECT: "direct", hs.HS_ALGO_TILED: "tiled"}
+    stream = torch.cuda.current_stream()
+
+    def step(events=None):
+        for v in variants:
+            if events is not None:
+                events[v][0].record(stream)
+            plans[v].hs_execute(x, sums, vmax, amax, stream)
+            if events is not None:
+                events[v][1].record(stream)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream, clocks sampled meanwhile --------------
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    per_step_events = [{v: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for v in variants}
+                       for _ in range(args.steps)]
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for k in range(args.steps):
+        step(per_step_events[k])
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    local_ms = ev0.elapsed_time(ev1)
+    total_ms = max_over_ranks_ms(local_ms, dist if world > 1 else None)
+    ms_per_step = total_ms / args.steps
+    bins_per_step = float(len(variants)) * batch * nbins * world
+    value = bins_per_step / (ms_per_step * 1e-3)
+
+    per_variant_ms = {v: statistics.mean(e[v][0].elapsed_time(e[v][1]) for e in per_step_events) for v in variants}
+    per_variant_best = {v: min(e[v][0].elapsed_time(e[v][1]) for e in per_step_events) for v in variants}
+    peak, peak_src = measured_peak()
+    bpb = BYTES_PER_BIN[out_mode]
+    per_variant = {}
+    for v in variants:
+        gbs = bpb * batch * nbins / (per_variant_ms[v] * 1e-3) / 1e9
+        per_variant[v] = {"ms": per_variant_ms[v], "best_ms": per_variant_best[v],
+                          "bins_per_s": batch * nbins / (per_variant_ms[v] * 1e-3), "eff_GBps": gbs,
+                          "frac_of_measured_peak": gbs / peak, "frac_of_nominal_8TBps": gbs / 8000.0,
+                          "algo": algo_names[plans[v].algo], "launches": plans[v].launches()}
+    dominant = max(variants, key=lambda v: per_variant_ms[v])
+    dom_algo = per_variant[dominant]["algo"]
+    roofline = {"bound": "hbm", "kernel": f"{dominant} ({dom_algo})", "achieved": per_variant[dominant]["eff_GBps"],
+                "peak": peak, "unit": "GB/s", "frac": per_variant[dominant]["eff_GBps"] / peak,
+                "traffic": ncu_traffic(dominant, args.workload, dom_algo),
+                "algorithmic_bytes_per_launch": bpb * batch * nbins, "peak_source": peak_src}
+
+    if rank != 0 and world > 1:
+        # other ranks still take part in the e2e collectives below
+        pass
+
+    # ---- e2e: the same step through hs_execute_host with pinned host buffers -------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        slab = max(1, min(batch, (1 << 26) // nbins))          # 256 MiB of input per slab
+        h_x = torch.empty((batch, nbins), dtype=torch.float32, pin_memory=True)
+        h_x.copy_(x)
+        h_sums = torch.empty((batch, L, nbins), dtype=torch.float32, pin_memory=True) if sums is not None else None
+        h_max = torch.empty((batch, nbins), dtype=torch.float32, pin_memory=True) if vmax is not None else None
+        h_amax = torch.empty((batch, nbins), dtype=torch.uint8, pin_memory=True) if amax is not None else None
+        stagings = {}
+        for v in variants:
+            st = torch.empty(plans[v].host_staging_bytes(slab), dtype=torch.uint8, device=dev)
+            plans[v].set_host_staging(st, slab)
+            stagings[v] = st
+
+        def host_step():
+            for v in variants:
+                plans[v].hs_execute_host(h_x, h_sums, h_max, h_amax, stream)
+
+        host_step()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.e2e_steps):
+            host_step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        wall_ms = (time.perf_counter() - t0) * 1e3
+        e2e_ms = max_over_ranks_ms(max(e0.elapsed_time(e1), wall_ms), dist if world > 1 else None) / args.e2e_steps
+        h2d = len(variants) * batch * nbins * 4
+        d2h = len(variants) * batch * nbins * (bpb - 4)
+        e2e = {"value": bins_per_step / (e2e_ms * 1e-3), "unit": "bins/s", "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": args.e2e_steps,
+               "slab_spectra": slab, "checksum_max": float(h_max[0, :16].sum()) if h_max is not None else None}
+        del stagings
+
+    # ---- cpu_baseline: the oracle on a bounded sample of the same workload (rank 0, N = 1 only) ------------------------
+    cpu = None
+    if rank == 0 and world == 1 and args.cpu_seconds > 0:
+        threads = os.cpu_count() or 1
+        rows = cpu_sample_rows(args.cpu_seconds, threads, nbins, variants)
+        rows = min(rows, batch)
+        x_rows = x[:rows].cpu().numpy()
+        rate, dt, done = oracle_rate(x_rows, variants, args.cpu_seconds, threads)
+        cpu = {"value": rate, "unit": "bins/s", "cores": threads, "kind": "oracle",
+               "sample": f"first {rows} spectra of the batch x {len(variants)} variants, whole spectra, {dt:.1f} s",
+               "gpu_over_cpu": value / rate}
+
+    if rank == 0:
+        line = {"metric": "harmonic_sum_bins_per_s", "value": value, "unit": "bins/s", "n_gpus": world,
+                "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_per_step,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": desc, "batch_per_gpu": batch, "nbins": nbins, "Hmax": 32, "out_mode": out_mode,
+                           "variants": variants, "algo": args.algo, "headline": not args.batch,
+                           "l2": f"input {batch * nbins * 4 / 2**20:.0f} MiB per variant launch vs 126 MB L2"
+                                 + ("" if batch * nbins * 4 > (1 << 28) else " (fits: not a headline size)"),
+                           "parallelism": f"dp{world} (batch shards, no collective)",
+                           "input_checksum_spectrum0": W.checksum(x[:1].cpu().numpy())},
+                "eff_GBps": value * bpb / 1e9 / world, "frac_of_measured_peak": value * bpb / 1e9 / world / peak,
+                "frac_of_nominal_8TBps": value * bpb / 1e9 / world / 8000.0,
+                "per_variant": per_variant, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+                "gpu_launches": sum(plans[v].launches() for v in variants) * args.steps, "clocks": clocks,
+                "paper_context": "PAPER.md:66-71 Table 1 GPU/CPU speed-ups 250x/704x/110x/177x (std/greedy/freq-bin/max), "
+                                 "hardware not stated"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,130 @@
+/*
+ * hs.h — C ABI of the batched incoherent harmonic sum for NVIDIA B200 (sm_100a).
+ *
+ * What is computed: for every spectrum b of a batch and every bin n, the partial harmonic sums
+ * h_H(n), H = 1,2,4,..,Hmax, of arXiv 1812.02647 (Adamek & Armour) in one of the paper's four variants
+ *     HS_STANDARD  eq. 1, PAPER.md:17      h_H(n) = H^-1/2 sum_{i=1..H} x(floor((n i + H/2)/H))
+ *     HS_MAX       eq. 2, PAPER.md:33      h_H(n) = H^-1/2 sum_{i=1..H} max_{0<=j<=i-1} x~(i n + j)
+ *     HS_FREQBIN   eq. 3, PAPER.md:38      h_H(n) = H^-1/2 sum_{i=1..H} x~(i n)
+ *     HS_GREEDY    eq. 4, PAPER.md:43-46   S_1 = x(n), j = 0; for i = 2..Hmax: l = x~(i n + j), r = x~(i n + j + 1),
+ *                                          S_i = S_{i-1} + max(l, r), j += (r > l);  h_H = H^-1/2 S_H
+ * with x~(k) = x(k) inside [0, nbins) and 0 outside.  The exact readings (rounding, window, tie and padding
+ * rules) are frozen in CONVENTIONS.md (C1..C11); the call names and argument order are fixed by
+ * BASELINE.json north_star.  The batch is data-parallel: spectra are independent.
+ *
+ * Layouts (row-major, all device pointers unless the name says host):
+ *     x       [batch][nbins]          float32   input, read-only, must not alias an output
+ *     sums    [batch][L][nbins]       float32   full output, plane l holds h_{2^l}; L = log2(Hmax)+1
+ *     max     [batch][nbins]          float32   reduced output: max over the L levels
+ *     argmax  [batch][nbins]          uint8     reduced output: smallest level index l in [0, L-1] attaining it
+ * Arithmetic: fp32 loads, fp32 accumulation, h = S * fp32(1/sqrt(H)); comparisons on raw fp32 values.
+ * Inputs must be finite (NaN/Inf: unspecified result, no fault).
+ *
+ * Ownership: the caller owns every buffer, including the workspace.  A plan owns host metadata only (and, once
+ * hs_plan_set_host_staging is called, three CUDA streams and their events).  No function allocates device memory.
+ * Errors: functions returning int return HS_OK (0) or an hs_status code; hs_plan_create returns NULL and records the
+ * code, readable with hs_last_error() (thread-local).  Nothing is printed, thrown or aborted across this ABI.
+ * There is no CPU fallback: without an sm_100 device hs_plan_create fails with HS_ERR_UNSUPPORTED.
+ */
+#ifndef HS_H
+#define HS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hs_plan hs_plan; /* opaque */
+
+enum hs_variant { HS_STANDARD = 0, HS_MAX = 1, HS_FREQBIN = 2, HS_GREEDY = 3 };
+enum hs_out_mode { HS_OUT_FULL = 1, HS_OUT_REDUCED = 2, HS_OUT_BOTH = 3 };
+enum hs_status {
+    HS_OK = 0,
+    HS_ERR_INVALID_ARG = 1,  /* a size, Hmax, variant, out_mode or option out of range                  */
+    HS_ERR_NULL_POINTER = 2, /* a required pointer is NULL                                              */
+    HS_ERR_MISALIGNED = 3,   /* a base pointer is not 16-byte aligned                                   */
+    HS_ERR_UNSUPPORTED = 4,  /* no CUDA device of compute capability 10.x is current                    */
+    HS_ERR_WORKSPACE = 5,    /* the chosen algorithm needs a workspace that was not set or is too small */
+    HS_ERR_CUDA = 6          /* a CUDA runtime call or kernel launch failed                             */
+};
+/* Kernel family.  HS_ALGO_AUTO picks the fastest one that is valid for the plan. */
+enum hs_algo {
+    HS_ALGO_AUTO = 0,
+    HS_ALGO_DIRECT = 1, /* one thread per output bin, loads straight from global memory; needs no workspace;
+                           every variant; kept as the simple on-device reference                              */
+    HS_ALGO_TILED = 2   /* the tuned kernels: eq. 1 staged windows in shared memory;
+                           eqs. 2-3 two-phase through an L2-resident workspace; eq. 4 staged blocks          */
+};
+
+/*
+ * hs_plan_create — describe one problem shape (the paper's statement of the problem: a batch of independent
+ * spectra; partial sums for an increasing number of harmonics; one algorithm of
+ * PAPER.md:17-46).
+ *   nbins    bins per spectrum, 4 <= nbins <= 2^25 and nbins % 4 == 0 (16-byte rows for vector/bulk copies; bin indices
+ *            up to 32*nbins+32 are int32)
+ *   batch    number of spectra, 1 <= batch, batch*nbins <= 2^40
+ *   Hmax     largest number of harmonics, one of 1,2,4,8,16,32
+ *   variant  enum hs_variant;  out_mode  enum hs_out_mode
+ * Does no device work.  Returns NULL on error: HS_ERR_INVALID_ARG (checked first), HS_ERR_UNSUPPORTED, HS_ERR_CUDA.
+ */
+hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode);
+
+/*
+ * hs_execute — enqueue the transform on `stream` (a cudaStream_t; NULL = the legacy default stream) and return
+ * without synchronising.  d_x, d_sums, d_max, d_argmax are DEVICE pointers in the layouts above.
+ * d_sums may be NULL iff out_mode lacks HS_OUT_FULL; d_max and d_argmax may be NULL iff it lacks HS_OUT_REDUCED;
+ * otherwise NULL -> HS_ERR_NULL_POINTER.  Base pointers must be 16-byte aligned -> HS_ERR_MISALIGNED.
+ * Every element of every requested output is overwritten.  A plan whose algorithm needs a workspace
+ * (hs_plan_workspace_bytes > 0) must have one set -> HS_ERR_WORKSPACE; such a plan must not be executed
+ * concurrently with itself.  Launch failure -> HS_ERR_CUDA.
+ */
+int hs_execute(const hs_plan *plan, const float *d_x, float *d_sums, float *d_max, uint8_t *d_argmax,
+               void *stream);
+
+/* hs_destroy — free the plan (host memory, and the staging streams if any).  NULL is a no-op returning HS_OK. */
+int hs_destroy(hs_plan *plan);
+
+/* ---- helpers ------------------------------------------------------------------------------------------------ */
+
+int hs_last_error(void);                 /* code of the last failed call on this thread (HS_OK if none)          */
+const char *hs_error_string(int code);   /* static string, never NULL                                            */
+const char *hs_version(void);            /* static string                                                        */
+
+int hs_plan_levels(const hs_plan *plan);                 /* L = log2(Hmax)+1, or -1 if plan is NULL               */
+int hs_plan_set_algo(hs_plan *plan, int algo);           /* enum hs_algo; resets the workspace requirement       */
+int hs_plan_algo(const hs_plan *plan);                   /* the resolved family (never HS_ALGO_AUTO), -1 if NULL */
+size_t hs_plan_workspace_bytes(const hs_plan *plan);     /* device scratch the resolved algorithm needs (0 = none) */
+/* d_ws: DEVICE pointer, 256-byte aligned, at least hs_plan_workspace_bytes(plan) bytes, owned by the caller and
+ * kept alive while the plan is executed.  Contents need no initialisation and are undefined afterwards. */
+int hs_plan_set_workspace(hs_plan *plan, void *d_ws, size_t bytes);
+/* Number of kernel launches (memset nodes included) one hs_execute of this plan enqueues; -1 if plan is NULL. */
+int hs_plan_launches(const hs_plan *plan);
+
+/*
+ * hs_execute_host — the same transform with HOST buffers (pinned memory recommended): h_x, h_sums, h_max, h_argmax
+ * are HOST pointers in the layouts above (NULL rules as hs_execute).  The batch is cut into slabs of spectra; each
+ * slab is copied to the device, transformed and copied back on one of three internal streams so that host->device
+ * copies, kernels and device->host copies overlap.  Work is ordered after what `stream` holds at the call and
+ * `stream` waits for it; the call itself does not synchronise.  Requires hs_plan_set_host_staging first.
+ */
+int hs_execute_host(hs_plan *plan, const float *h_x, float *h_sums, float *h_max, uint8_t *h_argmax,
+                    void *stream);
+/* Device bytes of staging hs_execute_host needs for slabs of `slab_spectra` spectra (3 slabs in flight, plus the
+ * algorithm's workspace per slab).  0 on error. */
+size_t hs_plan_host_staging_bytes(const hs_plan *plan, int64_t slab_spectra);
+/* d_staging: DEVICE pointer, 256-byte aligned, owned by the caller.  Creates the plan's streams and events. */
+int hs_plan_set_host_staging(hs_plan *plan, void *d_staging, size_t bytes, int64_t slab_spectra);
+
+/*
+ * hs_debug_greedy_paths — test-only: Greedy's drift j after each level, d_j[batch][L][nbins] uint8 (DEVICE),
+ * because BASELINE.json north_star asks for bit-exact j paths and the production outputs do not expose j.
+ * Valid for HS_GREEDY plans only (else HS_ERR_INVALID_ARG).  Not on the timed path.
+ */
+int hs_debug_greedy_paths(const hs_plan *plan, const float *d_x, uint8_t *d_j, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HS_H */

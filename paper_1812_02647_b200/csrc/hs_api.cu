@@ -1,0 +1,284 @@
+// hs_api.cu — the C ABI declared in include/hs.h: validation, plan bookkeeping, dispatch to the kernel families and
+// the host-buffer pipeline.  No torch types, no allocation of device memory, no output on stdout/stderr.
+#include <new>
+
+#include "hs_internal.cuh"
+
+namespace {
+thread_local int g_last_error = HS_OK;
+
+bool aligned(const void *p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+int levels_of(int Hmax)
+{
+    switch (Hmax) {
+        case 1: return 1;
+        case 2: return 2;
+        case 4: return 3;
+        case 8: return 4;
+        case 16: return 5;
+        case 32: return 6;
+        default: return -1;
+    }
+}
+
+void resolve_algo(hs_plan *p)
+{
+    if (p->algo_req == HS_ALGO_DIRECT) p->algo = HS_ALGO_DIRECT;
+    else if (p->algo_req == HS_ALGO_TILED) p->algo = HS_ALGO_TILED;
+    else p->algo = hs_tiled_supported(p) ? HS_ALGO_TILED : HS_ALGO_DIRECT;
+    p->ws = nullptr;
+    p->ws_bytes = 0;
+}
+
+int check_buffers(const hs_plan *p, const void *x, const void *sums, const void *vmax, const void *amax)
+{
+    if (!p || !x) HS_FAIL(HS_ERR_NULL_POINTER);
+    if ((p->out_mode & HS_OUT_FULL) && !sums) HS_FAIL(HS_ERR_NULL_POINTER);
+    if ((p->out_mode & HS_OUT_REDUCED) && (!vmax || !amax)) HS_FAIL(HS_ERR_NULL_POINTER);
+    if (!aligned(x, 16) || !aligned(sums, 16) || !aligned(vmax, 16) || !aligned(amax, 16)) HS_FAIL(HS_ERR_MISALIGNED);
+    return HS_OK;
+}
+
+int launch_family(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    if (p->algo == HS_ALGO_TILED && !buf.jdbg) return hs_launch_tiled(p, buf, batch, ws, stream);
+    return hs_launch_direct(p, buf, batch, ws, stream);
+}
+
+size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// bytes of one slab's device buffers in the host pipeline, each region 256-byte aligned
+struct slab_layout {
+    size_t x, sums, vmax, amax, ws, total;
+};
+slab_layout layout_of(const hs_plan *p, int64_t slab)
+{
+    slab_layout s{};
+    const size_t bins = (size_t)slab * (size_t)p->nbins;
+    s.x = round_up(bins * 4, 256);
+    s.sums = (p->out_mode & HS_OUT_FULL) ? round_up(bins * 4 * p->L, 256) : 0;
+    s.vmax = (p->out_mode & HS_OUT_REDUCED) ? round_up(bins * 4, 256) : 0;
+    s.amax = (p->out_mode & HS_OUT_REDUCED) ? round_up(bins, 256) : 0;
+    s.ws = p->algo == HS_ALGO_TILED ? round_up(hs_tiled_workspace_bytes(p, slab), 256) : 0;
+    s.total = s.x + s.sums + s.vmax + s.amax + s.ws;
+    return s;
+}
+}  // namespace
+
+void hs_set_error(int code) { g_last_error = code; }
+
+extern "C" {
+
+int hs_last_error(void) { return g_last_error; }
+
+const char *hs_error_string(int code)
+{
+    switch (code) {
+        case HS_OK: return "ok";
+        case HS_ERR_INVALID_ARG: return "invalid argument";
+        case HS_ERR_NULL_POINTER: return "required pointer is NULL";
+        case HS_ERR_MISALIGNED: return "pointer is not sufficiently aligned";
+        case HS_ERR_UNSUPPORTED: return "no CUDA device of compute capability 10.x (sm_100) is current";
+        case HS_ERR_WORKSPACE: return "workspace or staging buffer missing or too small";
+        case HS_ERR_CUDA: return "CUDA runtime call or kernel launch failed";
+        default: return "unknown hs_status code";
+    }
+}
+
+const char *hs_version(void) { return "hs 0.1 (sm_100a)"; }
+
+hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode)
+{
+    const int L = levels_of(Hmax);
+    if (nbins < 4 || nbins > ((int64_t)1 << 25) || (nbins % 4) != 0 || batch < 1 || L < 0 ||
+        variant < HS_STANDARD || variant > HS_GREEDY || out_mode < HS_OUT_FULL || out_mode > HS_OUT_BOTH ||
+        batch > ((int64_t)1 << 40) / nbins) {
+        hs_set_error(HS_ERR_INVALID_ARG);
+        return nullptr;
+    }
+    int dev = 0, major = 0, sms = 0, smem = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        hs_set_error(HS_ERR_UNSUPPORTED);
+        return nullptr;
+    }
+    if (major != 10) {
+        hs_set_error(HS_ERR_UNSUPPORTED);
+        return nullptr;
+    }
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        hs_set_error(HS_ERR_CUDA);
+        return nullptr;
+    }
+    hs_plan *p = new (std::nothrow) hs_plan();
+    if (!p) {
+        hs_set_error(HS_ERR_CUDA);
+        return nullptr;
+    }
+    p->nbins = nbins;
+    p->batch = batch;
+    p->Hmax = Hmax;
+    p->L = L;
+    p->variant = variant;
+    p->out_mode = out_mode;
+    p->algo_req = HS_ALGO_AUTO;
+    p->sm_count = sms;
+    p->smem_optin = (size_t)smem;
+    p->staging = nullptr;
+    p->staging_bytes = 0;
+    p->slab = 0;
+    p->lanes_ready = false;
+    resolve_algo(p);
+    return p;
+}
+
+int hs_destroy(hs_plan *p)
+{
+    if (!p) return HS_OK;
+    if (p->lanes_ready) {
+        for (int i = 0; i < HS_HOST_LANES; i++) {
+            cudaEventDestroy(p->lane_done[i]);
+            cudaStreamDestroy(p->lane_stream[i]);
+        }
+        cudaEventDestroy(p->fork);
+        (void)cudaGetLastError();
+    }
+    delete p;
+    return HS_OK;
+}
+
+int hs_plan_levels(const hs_plan *p) { return p ? p->L : -1; }
+int hs_plan_algo(const hs_plan *p) { return p ? p->algo : -1; }
+
+int hs_plan_set_algo(hs_plan *p, int algo)
+{
+    if (!p) HS_FAIL(HS_ERR_NULL_POINTER);
+    if (algo < HS_ALGO_AUTO || algo > HS_ALGO_TILED) HS_FAIL(HS_ERR_INVALID_ARG);
+    if (algo == HS_ALGO_TILED && !hs_tiled_supported(p)) HS_FAIL(HS_ERR_INVALID_ARG);
+    p->algo_req = algo;
+    resolve_algo(p);
+    return HS_OK;
+}
+
+size_t hs_plan_workspace_bytes(const hs_plan *p)
+{
+    if (!p) return 0;
+    return p->algo == HS_ALGO_TILED ? hs_tiled_workspace_bytes(p, p->batch) : 0;
+}
+
+int hs_plan_set_workspace(hs_plan *p, void *d_ws, size_t bytes)
+{
+    if (!p) HS_FAIL(HS_ERR_NULL_POINTER);
+    const size_t need = hs_plan_workspace_bytes(p);
+    if (need == 0) {
+        p->ws = d_ws;
+        p->ws_bytes = bytes;
+        return HS_OK;
+    }
+    if (!d_ws) HS_FAIL(HS_ERR_NULL_POINTER);
+    if (!aligned(d_ws, 256)) HS_FAIL(HS_ERR_MISALIGNED);
+    if (bytes < need) HS_FAIL(HS_ERR_WORKSPACE);
+    p->ws = d_ws;
+    p->ws_bytes = bytes;
+    return HS_OK;
+}
+
+int hs_plan_launches(const hs_plan *p)
+{
+    if (!p) return -1;
+    if (p->algo == HS_ALGO_TILED) return hs_tiled_launches(p, p->batch);
+    const int64_t tiles = (p->nbins + 255) / 256;
+    const int64_t max_spectra = ((int64_t)1 << 30) / tiles;
+    return (int)((p->batch + max_spectra - 1) / max_spectra);
+}
+
+int hs_execute(const hs_plan *p, const float *d_x, float *d_sums, float *d_max, uint8_t *d_argmax, void *stream)
+{
+    const int rc = check_buffers(p, d_x, d_sums, d_max, d_argmax);
+    if (rc != HS_OK) return rc;
+    if (hs_plan_workspace_bytes(p) > 0 && (!p->ws || p->ws_bytes < hs_plan_workspace_bytes(p))) HS_FAIL(HS_ERR_WORKSPACE);
+    hs_buffers buf{d_x, (p->out_mode & HS_OUT_FULL) ? d_sums : nullptr, (p->out_mode & HS_OUT_REDUCED) ? d_max : nullptr,
+                   (p->out_mode & HS_OUT_REDUCED) ? d_argmax : nullptr, nullptr};
+    return launch_family(p, buf, p->batch, p->ws, static_cast<cudaStream_t>(stream));
+}
+
+int hs_debug_greedy_paths(const hs_plan *p, const float *d_x, uint8_t *d_j, void *stream)
+{
+    if (!p || !d_x || !d_j) HS_FAIL(HS_ERR_NULL_POINTER);
+    if (p->variant != HS_GREEDY) HS_FAIL(HS_ERR_INVALID_ARG);
+    if (!aligned(d_x, 16) || !aligned(d_j, 16)) HS_FAIL(HS_ERR_MISALIGNED);
+    hs_buffers buf{d_x, nullptr, nullptr, nullptr, d_j};
+    return hs_launch_direct(p, buf, p->batch, nullptr, static_cast<cudaStream_t>(stream));
+}
+
+size_t hs_plan_host_staging_bytes(const hs_plan *p, int64_t slab)
+{
+    if (!p || slab < 1 || slab > p->batch) return 0;
+    return layout_of(p, slab).total * HS_HOST_LANES;
+}
+
+int hs_plan_set_host_staging(hs_plan *p, void *d_staging, size_t bytes, int64_t slab)
+{
+    if (!p || !d_staging) HS_FAIL(HS_ERR_NULL_POINTER);
+    if (slab < 1 || slab > p->batch) HS_FAIL(HS_ERR_INVALID_ARG);
+    if (!aligned(d_staging, 256)) HS_FAIL(HS_ERR_MISALIGNED);
+    if (bytes < hs_plan_host_staging_bytes(p, slab)) HS_FAIL(HS_ERR_WORKSPACE);
+    if (!p->lanes_ready) {
+        for (int i = 0; i < HS_HOST_LANES; i++) {
+            HS_CUDA_OK(cudaStreamCreateWithFlags(&p->lane_stream[i], cudaStreamNonBlocking));
+            HS_CUDA_OK(cudaEventCreateWithFlags(&p->lane_done[i], cudaEventDisableTiming));
+        }
+        HS_CUDA_OK(cudaEventCreateWithFlags(&p->fork, cudaEventDisableTiming));
+        p->lanes_ready = true;
+    }
+    p->staging = d_staging;
+    p->staging_bytes = bytes;
+    p->slab = slab;
+    return HS_OK;
+}
+
+int hs_execute_host(hs_plan *p, const float *h_x, float *h_sums, float *h_max, uint8_t *h_argmax, void *stream)
+{
+    if (!p || !h_x) HS_FAIL(HS_ERR_NULL_POINTER);
+    if ((p->out_mode & HS_OUT_FULL) && !h_sums) HS_FAIL(HS_ERR_NULL_POINTER);
+    if ((p->out_mode & HS_OUT_REDUCED) && (!h_max || !h_argmax)) HS_FAIL(HS_ERR_NULL_POINTER);
+    if (!p->lanes_ready || !p->staging) HS_FAIL(HS_ERR_WORKSPACE);
+    cudaStream_t user = static_cast<cudaStream_t>(stream);
+    const slab_layout lay = layout_of(p, p->slab);
+    const int64_t N = p->nbins;
+    HS_CUDA_OK(cudaEventRecord(p->fork, user));
+    for (int i = 0; i < HS_HOST_LANES; i++) HS_CUDA_OK(cudaStreamWaitEvent(p->lane_stream[i], p->fork, 0));
+    int lane = 0;
+    for (int64_t b0 = 0; b0 < p->batch; b0 += p->slab, lane = (lane + 1) % HS_HOST_LANES) {
+        const int64_t nb = (p->batch - b0 < p->slab) ? p->batch - b0 : p->slab;
+        const size_t bins = (size_t)nb * (size_t)N;
+        char *base = static_cast<char *>(p->staging) + (size_t)lane * lay.total;
+        float *dx = reinterpret_cast<float *>(base);
+        float *dsums = lay.sums ? reinterpret_cast<float *>(base + lay.x) : nullptr;
+        float *dmax = lay.vmax ? reinterpret_cast<float *>(base + lay.x + lay.sums) : nullptr;
+        uint8_t *damax = lay.amax ? reinterpret_cast<uint8_t *>(base + lay.x + lay.sums + lay.vmax) : nullptr;
+        void *dws = lay.ws ? base + lay.x + lay.sums + lay.vmax + lay.amax : nullptr;
+        cudaStream_t s = p->lane_stream[lane];
+        HS_CUDA_OK(cudaMemcpyAsync(dx, h_x + (size_t)b0 * N, bins * 4, cudaMemcpyHostToDevice, s));
+        hs_buffers buf{dx, dsums, dmax, damax, nullptr};
+        const int rc = launch_family(p, buf, nb, dws, s);
+        if (rc != HS_OK) return rc;
+        if (dsums)
+            HS_CUDA_OK(cudaMemcpyAsync(h_sums + (size_t)b0 * p->L * N, dsums, bins * 4 * p->L, cudaMemcpyDeviceToHost, s));
+        if (dmax) {
+            HS_CUDA_OK(cudaMemcpyAsync(h_max + (size_t)b0 * N, dmax, bins * 4, cudaMemcpyDeviceToHost, s));
+            HS_CUDA_OK(cudaMemcpyAsync(h_argmax + (size_t)b0 * N, damax, bins, cudaMemcpyDeviceToHost, s));
+        }
+    }
+    for (int i = 0; i < HS_HOST_LANES; i++) {
+        HS_CUDA_OK(cudaEventRecord(p->lane_done[i], p->lane_stream[i]));
+        HS_CUDA_OK(cudaStreamWaitEvent(user, p->lane_done[i], 0));
+    }
+    return HS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,95 @@
+// hs_internal.cuh — plan layout, error plumbing and the shared device-side epilogue (normalise, full planes,
+// running max/argmax).  Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/hs.h"
+
+#define HS_MAX_LEVELS 6
+#define HS_HOST_LANES 3
+
+struct hs_plan {
+    int64_t nbins, batch;
+    int Hmax, L, variant, out_mode;
+    int algo_req;  // what the caller asked for (enum hs_algo)
+    int algo;      // resolved family, never AUTO
+    int sm_count;
+    size_t smem_optin;  // max dynamic shared memory per block
+    // workspace for the resolved algorithm (device, caller-owned)
+    void *ws;
+    size_t ws_bytes;
+    // host-buffer path (hs_execute_host)
+    void *staging;
+    size_t staging_bytes;
+    int64_t slab;
+    cudaStream_t lane_stream[HS_HOST_LANES];
+    cudaEvent_t lane_done[HS_HOST_LANES];
+    cudaEvent_t fork;
+    bool lanes_ready;
+};
+
+// ---- error plumbing (hs_api.cu) ---------------------------------------------------------------------------------
+void hs_set_error(int code);
+#define HS_FAIL(code)          \
+    do {                       \
+        hs_set_error(code);    \
+        return (code);         \
+    } while (0)
+#define HS_CUDA_OK(expr)                        \
+    do {                                        \
+        if ((expr) != cudaSuccess) {            \
+            (void)cudaGetLastError();           \
+            HS_FAIL(HS_ERR_CUDA);               \
+        }                                       \
+    } while (0)
+
+// ---- launch entry points of the kernel families -------------------------------------------------------------------
+// Each enqueues on `stream` for spectra [0, batch) of the given buffers and returns an hs_status.
+struct hs_buffers {
+    const float *x;
+    float *sums;
+    float *vmax;
+    uint8_t *amax;
+    uint8_t *jdbg;  // Greedy debug paths or nullptr
+};
+int hs_launch_direct(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
+int hs_launch_tiled(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
+size_t hs_tiled_workspace_bytes(const hs_plan *p, int64_t batch);
+int hs_tiled_launches(const hs_plan *p, int64_t batch);
+bool hs_tiled_supported(const hs_plan *p);
+
+// ---- device-side epilogue ---------------------------------------------------------------------------------------
+// c_H = fp32(1/sqrt(H)) for H = 1,2,4,8,16,32 (CONVENTIONS.md C7; "1/sqrt(H)").
+__device__ __forceinline__ constexpr float hs_norm(int l)
+{
+    return l == 0 ? 1.0f
+         : l == 1 ? 0.70710678118654752440f
+         : l == 2 ? 0.5f
+         : l == 3 ? 0.35355339059327376220f
+         : l == 4 ? 0.25f
+                  : 0.17677669529663688110f;
+}
+
+// Running reduced output of one bin: m = max_l h_l, a = smallest l attaining it (C8).
+template <int OUT>
+struct hs_emit {
+    float m;
+    int a;
+    // plane0 points at sums[b][0][n]; consecutive levels are `N` floats apart.
+    __device__ __forceinline__ void level(int l, float S, float *__restrict__ plane0, int64_t N)
+    {
+        const float h = S * hs_norm(l);
+        if (OUT & HS_OUT_FULL) plane0[(int64_t)l * N] = h;
+        if (OUT & HS_OUT_REDUCED) {
+            if (l == 0) {
+                m = h;
+                a = 0;
+            } else if (h > m) {
+                m = h;
+                a = l;
+            }
+        }
+    }
+};

@@ -1,0 +1,285 @@
+"""Parity of the CUDA path (through the C ABI, include/hs.h) with the oracle, element by element on the same seeded
+inputs.  Tolerances are those of BASELINE.json north_star / CONVENTIONS.md C10:
+    sums and maxima  |gpu - ref| <= 1e-5 (1 + |ref|);   Greedy j exact;
+    best level exact unless the oracle's top two levels differ by less than the tolerance.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from parity import argmax_from_levels, check_argmax, check_sums
+
+pytestmark = pytest.mark.gpu
+
+VARIANTS = ["standard", "max", "freqbin", "greedy"]
+ALGOS = ["direct", "tiled"]
+
+
+@pytest.fixture(scope="module")
+def hs():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1812_02647_b200 import build
+    build.build()
+    import paper_1812_02647_b200.binding as binding
+    return binding
+
+
+def make_plan(hs, N, B, Hmax, variant, out_mode, algo):
+    plan = hs.hs_plan_create(N, B, Hmax, variant, out_mode)
+    if algo == "tiled":
+        try:
+            plan.set_algo("tiled")
+        except hs.HsError:
+            pytest.skip("no tuned kernel covers this plan")
+    else:
+        plan.set_algo(algo)
+    return plan
+
+
+def run_and_compare(hs, oracle, x_np, Hmax, variant, out_mode, algo, check_j=True):
+    """Run the whole batch on the GPU and compare every element with the oracle."""
+    B, N = x_np.shape
+    d_x = torch.from_numpy(x_np).cuda()
+    plan = make_plan(hs, N, B, Hmax, variant, out_mode, algo)
+    sums, vmax, amax = plan.run(d_x)
+    torch.cuda.synchronize()
+    ref = oracle.harmonic_sum(x_np, Hmax, variant, want_jpath=(variant == "greedy"))
+    what = f"{variant}/{algo}/{out_mode}/N={N}/B={B}/Hmax={Hmax}"
+    if sums is not None:
+        check_sums(sums.cpu().numpy(), ref["sums"], what + " sums")
+        np.testing.assert_array_equal(sums[:, 0].cpu().numpy(), x_np)               # h_1(n) = x(n) bit-exactly
+    if vmax is not None:
+        check_sums(vmax.cpu().numpy(), ref["max"], what + " max")
+        check_argmax(amax.cpu().numpy(), ref["argmax"], ref["second"], ref["gap"], ref["max"], what + " argmax")
+    if sums is not None and vmax is not None:                                        # P13: max is one of the planes
+        pick = torch.gather(sums, 1, amax.long().unsqueeze(1)).squeeze(1)
+        assert torch.equal(pick, vmax), what + " max != sums[argmax]"
+    if variant == "greedy" and check_j:
+        d_j = torch.empty((B, plan.levels, N), dtype=torch.uint8, device="cuda")
+        plan.hs_debug_greedy_paths(d_x, d_j)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(d_j.cpu().numpy(), ref["jpath"])
+    plan.hs_destroy()
+
+
+# ---------------------------------------------------------------------------------------------------- small and ragged
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_small_and_ragged_sizes(hs, oracle, variant, algo):
+    rng = np.random.default_rng(1)
+    for N, B in ((4, 1), (8, 3), (12, 1), (36, 2), (100, 1), (1000, 3), (4100, 2), (33000, 1)):
+        x = (rng.standard_exponential((B, N)) - 1).astype(np.float32)
+        run_and_compare(hs, oracle, x, 32, variant, "both", algo)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_every_hmax_and_out_mode(hs, oracle, variant, algo):
+    rng = np.random.default_rng(2)
+    x = rng.standard_normal((2, 20000)).astype(np.float32)
+    for Hmax in (1, 2, 4, 8, 16, 32):
+        for out_mode in ("full", "reduced", "both"):
+            run_and_compare(hs, oracle, x, Hmax, variant, out_mode, algo, check_j=(out_mode == "full"))
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_degenerate_spectra(hs, oracle, variant, algo):
+    N = 6000
+    rng = np.random.default_rng(3)
+    cases = [np.zeros(N), -np.ones(N), np.ones(N), np.arange(N), np.arange(N)[::-1],
+             rng.integers(-2, 3, N), np.where(np.arange(N) % 7 == 0, 5.0, -1.0)]
+    x = np.stack(cases).astype(np.float32)
+    run_and_compare(hs, oracle, x, 32, variant, "both", algo)
+    # all levels tie on the zero spectrum: the smallest level wins (C8)
+    plan = make_plan(hs, N, 1, 32, variant, "reduced", algo)
+    _, vmax, amax = plan.run(torch.zeros((1, N), device="cuda"))
+    assert int(amax.max()) == 0 and float(vmax.abs().max()) == 0.0
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_integer_bin_comb_all_variants_agree(hs, algo):
+    N, m = 1 << 16, 1251
+    a = (10.0 * 0.9 ** np.arange(32) + 0.5).astype(np.float32)
+    x = np.zeros((1, N), np.float32)
+    x[0, m * np.arange(1, 33)] = a
+    d_x = torch.from_numpy(x).cuda()
+    vals = {}
+    for v in VARIANTS:
+        sums, _, _ = make_plan(hs, N, 1, 32, v, "full", algo).run(d_x)
+        vals[v] = sums[0].cpu().numpy()
+    for l, H in enumerate((1, 2, 4, 8, 16, 32)):
+        ref = float(np.cumsum(a.astype(np.float64))[H - 1] / math.sqrt(H))
+        assert vals["standard"][l, H * m] == pytest.approx(ref, rel=1e-5)
+        for v in ("max", "freqbin", "greedy"):
+            assert vals[v][l, m] == pytest.approx(ref, rel=1e-5)
+
+
+# ---------------------------------------------------------------------------------------------------- configs 0 and 1
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config0_full_output(hs, oracle, variant, algo):
+    run_and_compare(hs, oracle, W.config0(), 32, variant, "full", algo)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config1_subset_full_and_reduced(hs, oracle, variant, algo):
+    flags = [W.rng_for(1, b).random() < 0.10 for b in range(256)]
+    chosen = [b for b in range(256) if flags[b]][:2] + [0, 255]
+    x, _ = W.config1(chosen)
+    run_and_compare(hs, oracle, x, 32, variant, "both", algo, check_j=False)
+
+
+# ---------------------------------------------------------------------------------------------------- full-size configs
+def sampled_compare(hs, oracle, d_x, variant, out_mode, algo, spectra, npoints, seed):
+    """At sizes the oracle cannot cover: launch on the whole batch exactly as bench.py does, then compare sampled
+    outputs (whole rows of a few spectra's low bins plus random points) computed one by one by the oracle."""
+    B, N = d_x.shape
+    plan = make_plan(hs, N, B, 32, variant, out_mode, algo)
+    sums, vmax, amax = plan.run(d_x)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(seed)
+    bidx = np.concatenate([rng.choice(spectra, npoints), np.repeat(spectra[:4], 64)])
+    nidx = np.concatenate([rng.integers(0, N, npoints), np.tile(np.arange(64), len(spectra[:4]))])
+    # low bins (all 32 harmonics in range) are a tiny fraction of uniform samples: add some explicitly
+    extra = npoints // 4
+    bidx = np.concatenate([bidx, rng.choice(spectra, extra)])
+    nidx = np.concatenate([nidx, rng.integers(0, N // 32, extra)])
+    rows = sorted(set(int(b) for b in bidx))
+    x_rows = d_x[rows].cpu().numpy()
+    remap = {b: i for i, b in enumerate(rows)}
+    h, _ = oracle.points(x_rows, 32, variant, np.array([remap[int(b)] for b in bidx]), nidx)
+    tb, tn = torch.as_tensor(bidx, device="cuda"), torch.as_tensor(nidx, device="cuda")
+    what = f"{variant}/{algo}/{out_mode} sampled B={B} N={N}"
+    if sums is not None:
+        check_sums(sums[tb, :, tn].cpu().numpy(), h, what + " sums")
+    if vmax is not None:
+        best, second, gap, m = argmax_from_levels(h)
+        check_sums(vmax[tb, tn].cpu().numpy(), m, what + " max")
+        check_argmax(amax[tb, tn].cpu().numpy(), best, second, gap, m, what + " argmax")
+        assert int(amax.max()) <= 5
+    # properties that hold at any size: h_1 = x, and the reduced maximum is at least x
+    if sums is not None:
+        assert torch.equal(sums[:, 0], d_x)
+    if vmax is not None:
+        assert bool((vmax >= d_x).all())
+    plan.hs_destroy()
+    del sums, vmax, amax
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_config2_full_size_reduced_sampled(hs, oracle, algo):
+    d_x, injected = W.config2_torch("cuda")
+    assert d_x.shape == (4096, 1 << 18) and 20 <= len(injected) <= 70
+    spectra = np.array(sorted(set(injected[:12] + [0, 4095] + list(range(64, 4096, 512)))))
+    for v in VARIANTS:
+        sampled_compare(hs, oracle, d_x, v, "reduced", algo, spectra, 4000, 22)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_config3_long_spectra_full_output_sampled(hs, oracle, algo):
+    d_x, injected = W.config3_torch("cuda")
+    assert d_x.shape == (8, 1 << 23) and len(injected) == 8
+    for v in VARIANTS:
+        sampled_compare(hs, oracle, d_x, v, "full", algo, np.arange(8), 3000, 33)
+
+
+@pytest.mark.parametrize("algo", ALGOS)
+def test_scaling_shapes_short_and_long_spectra(hs, oracle, algo):
+    # configs[4] scaling sweep shapes, shrunk in batch: 2^16-bin and 2^24-bin spectra, Hmax 8 and 32
+    for N, B in ((1 << 16, 64), (1 << 24, 2)):
+        d_x = W.exp_noise_torch(B, N, 4, "cuda")
+        for v in VARIANTS:
+            sampled_compare(hs, oracle, d_x, v, "reduced", algo, np.arange(min(B, 8)), 1500, 44)
+
+
+# ---------------------------------------------------------------------------------------------------- ABI behaviour on the device
+def test_error_paths_on_device(hs):
+    plan = hs.hs_plan_create(1024, 2, 32, "max", "both")
+    x = torch.zeros((2, 1024), device="cuda")
+    sums = torch.empty((2, 6, 1024), device="cuda")
+    vmax = torch.empty((2, 1024), device="cuda")
+    amax = torch.empty((2, 1024), dtype=torch.uint8, device="cuda")
+    plan.ensure_workspace()
+    with pytest.raises(hs.HsError) as e:
+        plan.hs_execute(x, None, vmax, amax)
+    assert e.value.code == hs.HS_ERR_NULL_POINTER
+    with pytest.raises(hs.HsError) as e:
+        plan.hs_execute(x, sums, vmax, None)
+    assert e.value.code == hs.HS_ERR_NULL_POINTER
+    off = torch.zeros(2 * 1024 + 1, device="cuda")[1:].view(2, 1024)
+    with pytest.raises(hs.HsError) as e:
+        plan.hs_execute(off, sums, vmax, amax)
+    assert e.value.code == hs.HS_ERR_MISALIGNED
+    plan.hs_execute(x, sums, vmax, amax)
+    torch.cuda.synchronize()
+    g = hs.hs_plan_create(1024, 2, 32, "standard", "full")
+    with pytest.raises(hs.HsError) as e:
+        g.hs_debug_greedy_paths(x, amax)
+    assert e.value.code == hs.HS_ERR_INVALID_ARG
+    assert plan.launches() >= 1 and plan.levels == 6
+    with pytest.raises(hs.HsError):
+        plan.set_algo(7)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_workspace_is_required_when_the_algorithm_needs_one(hs, variant):
+    plan = hs.hs_plan_create(1 << 14, 4, 32, variant, "reduced")
+    if plan.workspace_bytes() == 0:
+        return
+    x = torch.zeros((4, 1 << 14), device="cuda")
+    vmax = torch.empty((4, 1 << 14), device="cuda")
+    amax = torch.empty((4, 1 << 14), dtype=torch.uint8, device="cuda")
+    with pytest.raises(hs.HsError) as e:
+        plan.hs_execute(x, None, vmax, amax)
+    assert e.value.code == hs.HS_ERR_WORKSPACE
+    small = torch.empty(256, dtype=torch.uint8, device="cuda")
+    with pytest.raises(hs.HsError) as e:
+        plan.set_workspace(small)
+    assert e.value.code == hs.HS_ERR_WORKSPACE
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_non_default_stream_and_repeat_calls(hs, oracle, variant):
+    rng = np.random.default_rng(9)
+    x = (rng.standard_exponential((5, 50000)) - 1).astype(np.float32)
+    d_x = torch.from_numpy(x).cuda()
+    plan = hs.hs_plan_create(50000, 5, 32, variant, "reduced")
+    plan.ensure_workspace()
+    vmax = torch.empty((5, 50000), device="cuda")
+    amax = torch.empty((5, 50000), dtype=torch.uint8, device="cuda")
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        for _ in range(3):                                   # the workspace is reused across calls
+            vmax.fill_(float("nan"))
+            plan.hs_execute(d_x, None, vmax, amax, stream=s)
+    s.synchronize()
+    ref = oracle.harmonic_sum(x, 32, variant, want_sums=False)
+    check_sums(vmax.cpu().numpy(), ref["max"], variant + " stream max")
+    check_argmax(amax.cpu().numpy(), ref["argmax"], ref["second"], ref["gap"], ref["max"], variant + " stream argmax")
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("out_mode", ["reduced", "both"])
+def test_host_buffer_entry_matches_device_entry(hs, variant, out_mode):
+    B, N, slab = 11, 1 << 15, 4                               # ragged last slab, more slabs than lanes
+    x = W.exp_noise_torch(B, N, 5, "cpu").pin_memory()
+    plan = hs.hs_plan_create(N, B, 32, variant, out_mode)
+    sums_d, vmax_d, amax_d = plan.run(x.cuda())
+    staging = torch.empty(plan.host_staging_bytes(slab), dtype=torch.uint8, device="cuda")
+    plan.set_host_staging(staging, slab)
+    h_sums = torch.empty((B, 6, N), dtype=torch.float32).pin_memory() if out_mode == "both" else None
+    h_max = torch.empty((B, N), dtype=torch.float32).pin_memory()
+    h_amax = torch.empty((B, N), dtype=torch.uint8).pin_memory()
+    plan.hs_execute_host(x, h_sums, h_max, h_amax)
+    torch.cuda.synchronize()
+    assert torch.equal(h_max, vmax_d.cpu()) and torch.equal(h_amax, amax_d.cpu())
+    if h_sums is not None:
+        assert torch.equal(h_sums, sums_d.cpu())
