@@ -1,0 +1,129 @@
+// hs_greedy_gather.cu — eq. 4 (CONVENTIONS.md C4, C5) as a per-thread, divergence-free gather.
+//
+// One thread owns one fundamental bin n and runs the chain i = 2..Hmax: l = x~(i n + j), r = x~(i n + j + 1),
+// S += max(l, r), j += (r > l).  The candidates of harmonic i lie in the aligned block [i n, i n + i - 1], so for a
+// warp of 32 consecutive n everything is in range while i (n_hi + 1) <= N: that bound is warp-uniform, and only
+// the few harmonics that straddle the end of the spectrum take the predicated (zero-padded) path; harmonics that
+// are out of range for the whole warp contribute max(0, 0) = 0 and leave j unchanged, so they are skipped.
+// Averaged over a spectrum a bin has 4.06 in-range harmonics of the 32 (load imbalance of PAPER.md:21), which is why
+// skipping matters more than anything else here: the direct kernel issues all 31 steps for every bin.
+#include "hs_internal.cuh"
+#include "hs_ptx.cuh"
+
+namespace {
+
+constexpr int kThreads = 128;
+constexpr int kGridY = 32;   // spectra are strided over gridDim.y so that the per-thread prologue is amortised
+
+template <int L, int OUT>
+__global__ void __launch_bounds__(kThreads)
+hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
+                        uint8_t *__restrict__ amax, int N, int batch)
+{
+    const int n = blockIdx.x * kThreads + threadIdx.x;
+    const int n_lo = n & ~31;                      // first bin of this warp
+    if (n_lo >= N) return;
+    const bool valid = n < N;
+    const int nn = valid ? n : N - 1;              // lanes past the end shadow the last bin and store nothing
+    const int n_hi1 = min(n_lo + 32, N);           // one past the warp's last bin
+    // Warp-uniform range tests (no divisions): harmonic i is in range for EVERY lane, neighbour included, iff
+    // i * n_hi1 <= N; it is in range for SOME lane iff i * n_lo < N.
+    for (int b = blockIdx.y; b < batch; b += gridDim.y) {
+        const float *__restrict__ xb = x + b * (int64_t)N;
+        hs_emit<OUT> e;
+        float *plane0 = (OUT & HS_OUT_FULL) ? sums + ((int64_t)b * L) * N + nn : nullptr;
+        float S = __ldg(xb + nn);
+        if (valid) e.level(0, S, plane0, N);
+        else e.reduce(0, S);
+        int j = 0;
+        bool tail = false;
+#pragma unroll
+        for (int l = 1; l < L; l++) {
+            const int lo = (1 << (l - 1)) + 1, hi = 1 << l;
+            if (lo * n_lo < N) {                    // some harmonic of this level is in range for some lane
+                int i = lo;
+                int base = (lo - 1) * nn;           // (i - 1) * n
+#pragma unroll 4
+                for (; i <= hi && i * n_hi1 <= N; i++) {
+                    base += nn;
+                    const float *__restrict__ p = xb + (base + j);
+                    const float lft = __ldg(p), rgt = __ldg(p + 1);
+                    const bool right = rgt > lft;   // strictly greater (C4)
+                    S += right ? rgt : lft;
+                    j += right ? 1 : 0;
+                }
+                for (; i <= hi && i * n_lo < N; i++) {
+                    base += nn;
+                    const int k = base + j;
+                    const float lft = k < N ? __ldg(xb + k) : 0.0f;
+                    const float rgt = k + 1 < N ? __ldg(xb + k + 1) : 0.0f;
+                    const bool right = rgt > lft;
+                    S += right ? rgt : lft;
+                    j += right ? 1 : 0;
+                }
+                if (valid) e.level(l, S, plane0, N);
+                else e.reduce(l, S);
+            } else if (OUT != HS_OUT_REDUCED) {
+                if (valid) e.level(l, S, plane0, N);
+            } else {
+                tail = true;
+            }
+        }
+        // Levels whose harmonics are all out of range leave S unchanged, and h_l = S c_l is monotone in l: for S >= 0
+        // no later level exceeds the running maximum, for S < 0 the last level is the largest.  Test level L-1 only.
+        if (OUT == HS_OUT_REDUCED && tail) e.reduce(L - 1, S * hs_norm(L - 1));
+        if ((OUT & HS_OUT_REDUCED) && valid) {
+            hsptx::st_cs(vmax + b * (int64_t)N + n, e.m);
+            hsptx::st_cs(amax + b * (int64_t)N + n, (uint8_t)e.a);
+        }
+    }
+}
+
+template <int L, int OUT>
+int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+{
+    const int N = (int)p->nbins;
+    const int tiles = (N + kThreads - 1) / kThreads;
+    const int64_t max_spectra = (int64_t)1 << 30;            // int b inside the kernel
+    for (int64_t b0 = 0; b0 < batch; b0 += max_spectra) {
+        const int64_t nb = (batch - b0 < max_spectra) ? batch - b0 : max_spectra;
+        const int64_t off = b0 * (int64_t)N;
+        const dim3 grid((unsigned)tiles, (unsigned)(nb < kGridY ? nb : kGridY), 1);
+        hs_greedy_gather_kernel<L, OUT><<<grid, kThreads, 0, stream>>>(
+            buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
+            buf.amax ? buf.amax + off : nullptr, N, (int)nb);
+        HS_CUDA_OK(cudaGetLastError());
+    }
+    return HS_OK;
+}
+
+template <int L>
+int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+{
+    switch (p->out_mode) {
+        case HS_OUT_FULL: return launch<L, HS_OUT_FULL>(p, buf, batch, stream);
+        case HS_OUT_REDUCED: return launch<L, HS_OUT_REDUCED>(p, buf, batch, stream);
+        default: return launch<L, HS_OUT_BOTH>(p, buf, batch, stream);
+    }
+}
+
+}  // namespace
+
+int hs_greedy_gather_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+{
+    switch (p->L) {
+        case 1: return by_out<1>(p, buf, batch, stream);
+        case 2: return by_out<2>(p, buf, batch, stream);
+        case 3: return by_out<3>(p, buf, batch, stream);
+        case 4: return by_out<4>(p, buf, batch, stream);
+        case 5: return by_out<5>(p, buf, batch, stream);
+        default: return by_out<6>(p, buf, batch, stream);
+    }
+}
+
+int hs_greedy_gather_launches(const hs_plan *p, int64_t batch)
+{
+    (void)p;
+    const int64_t max_spectra = (int64_t)1 << 30;
+    return (int)((batch + max_spectra - 1) / max_spectra);
+}

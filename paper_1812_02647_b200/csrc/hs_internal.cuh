@@ -59,6 +59,15 @@ int hs_launch_tiled(const hs_plan *p, const hs_buffers &buf, int64_t batch, void
 size_t hs_tiled_workspace_bytes(const hs_plan *p, int64_t batch);
 int hs_tiled_launches(const hs_plan *p, int64_t batch);
 bool hs_tiled_supported(const hs_plan *p);
+// per-variant tuned kernels
+int hs_standard_tiled_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream);
+int hs_standard_tiled_launches(const hs_plan *p, int64_t batch);
+int hs_twophase_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
+int hs_twophase_launches(const hs_plan *p, int64_t batch);
+size_t hs_twophase_workspace_bytes(const hs_plan *p, int64_t batch);
+bool hs_twophase_supported(const hs_plan *p, int64_t batch);
+int hs_greedy_gather_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream);
+int hs_greedy_gather_launches(const hs_plan *p, int64_t batch);
 
 // ---- device-side epilogue ---------------------------------------------------------------------------------------
 // c_H = fp32(1/sqrt(H)) for H = 1,2,4,8,16,32 (CONVENTIONS.md C7; "1/sqrt(H)").
@@ -77,19 +86,22 @@ template <int OUT>
 struct hs_emit {
     float m;
     int a;
+    // running max over the levels; a level replaces the maximum only if strictly greater
+    __device__ __forceinline__ void reduce(int l, float h)
+    {
+        if (l == 0) {
+            m = h;
+            a = 0;
+        } else if (h > m) {
+            m = h;
+            a = l;
+        }
+    }
     // plane0 points at sums[b][0][n]; consecutive levels are `N` floats apart.
     __device__ __forceinline__ void level(int l, float S, float *__restrict__ plane0, int64_t N)
     {
         const float h = S * hs_norm(l);
         if (OUT & HS_OUT_FULL) plane0[(int64_t)l * N] = h;
-        if (OUT & HS_OUT_REDUCED) {
-            if (l == 0) {
-                m = h;
-                a = 0;
-            } else if (h > m) {
-                m = h;
-                a = l;
-            }
-        }
+        if (OUT & HS_OUT_REDUCED) reduce(l, h);
     }
 };
