@@ -54,8 +54,9 @@ enum hs_algo {
     HS_ALGO_AUTO = 0,
     HS_ALGO_DIRECT = 1, /* one thread per output bin, loads straight from global memory; needs no workspace;
                            every variant; kept as the simple on-device reference                              */
-    HS_ALGO_TILED = 2   /* the tuned kernels: eq. 1 staged windows in shared memory;
-                           eqs. 2-3 two-phase through an L2-resident workspace; eq. 4 staged blocks          */
+    HS_ALGO_TILED = 2,  /* the tuned kernels: eq. 1 windows staged in shared memory by TMA;
+                           eq. 2 two-phase through an L2-resident workspace; eqs. 3-4 range-skipping gather         */
+    HS_ALGO_TWOPHASE = 3 /* eqs. 2-3 only: the two-phase kernel (for eq. 2 the same as HS_ALGO_TILED)               */
 };
 
 /*

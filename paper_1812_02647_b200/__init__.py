@@ -5,7 +5,7 @@ The product is the C-ABI library libhs.so (include/hs.h, csrc/); this package is
 Attribute access is lazy so that `python -m paper_1812_02647_b200.build` works before libhs.so exists; touching
 any binding name without the library raises ImportError (there is no CPU fallback).
 """
-_BINDING_NAMES = ("ALGOS", "HS_ALGO_AUTO", "HS_ALGO_DIRECT", "HS_ALGO_TILED", "HS_FREQBIN", "HS_GREEDY", "HS_MAX",
+_BINDING_NAMES = ("ALGOS", "HS_ALGO_AUTO", "HS_ALGO_DIRECT", "HS_ALGO_TILED", "HS_ALGO_TWOPHASE", "HS_FREQBIN", "HS_GREEDY", "HS_MAX",
                   "HS_OUT_BOTH", "HS_OUT_FULL", "HS_OUT_REDUCED", "HS_STANDARD", "LIB_PATH", "OUT_MODES", "VARIANTS",
                   "HsError", "Plan", "hs_plan_create", "lib")
 

@@ -15,8 +15,8 @@ namespace {
 constexpr int kThreads = 128;
 constexpr int kGridY = 32;   // spectra are strided over gridDim.y so that the per-thread prologue is amortised
 
-template <int L, int OUT>
-__global__ void __launch_bounds__(kThreads)
+template <int VARIANT, int L, int OUT>
+__global__ void __launch_bounds__(kThreads, 12)
 hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
                         uint8_t *__restrict__ amax, int N, int batch)
 {
@@ -43,23 +43,42 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
             if (lo * n_lo < N) {                    // some harmonic of this level is in range for some lane
                 int i = lo;
                 int base = (lo - 1) * nn;           // (i - 1) * n
-#pragma unroll 4
-                for (; i <= hi && i * n_hi1 <= N; i++) {
-                    base += nn;
-                    const float *__restrict__ p = xb + (base + j);
-                    const float lft = __ldg(p), rgt = __ldg(p + 1);
-                    const bool right = rgt > lft;   // strictly greater (C4)
-                    S += right ? rgt : lft;
-                    j += right ? 1 : 0;
-                }
-                for (; i <= hi && i * n_lo < N; i++) {
-                    base += nn;
-                    const int k = base + j;
-                    const float lft = k < N ? __ldg(xb + k) : 0.0f;
-                    const float rgt = k + 1 < N ? __ldg(xb + k + 1) : 0.0f;
-                    const bool right = rgt > lft;
-                    S += right ? rgt : lft;
-                    j += right ? 1 : 0;
+                if (VARIANT == HS_FREQBIN && hi * n_hi1 <= N) {   // whole level in range for every lane: fixed trip count
+                    {    // eq. 3: x(i n); the loads are independent and all in flight at once
+                        float v[16];
+#pragma unroll
+                        for (int q = 0; q < 16; q++)
+                            if (q <= hi - lo) v[q] = __ldg(xb + (lo + q) * nn);
+#pragma unroll
+                        for (int q = 0; q < 16; q++)
+                            if (q <= hi - lo) S += v[q];
+                    }
+                } else {
+                    for (; i <= hi && i * n_hi1 <= N; i++) {
+                        base += nn;
+                        if (VARIANT == HS_FREQBIN) {
+                            S += __ldg(xb + base);
+                        } else {
+                            const float *__restrict__ p = xb + (base + j);
+                            const float lft = __ldg(p), rgt = __ldg(p + 1);
+                            const bool right = rgt > lft;
+                            S += right ? rgt : lft;
+                            j += right ? 1 : 0;
+                        }
+                    }
+                    for (; i <= hi && i * n_lo < N; i++) {
+                        base += nn;
+                        if (VARIANT == HS_FREQBIN) {
+                            S += base < N ? __ldg(xb + base) : 0.0f;
+                        } else {
+                            const int k = base + j;
+                            const float lft = k < N ? __ldg(xb + k) : 0.0f;
+                            const float rgt = k + 1 < N ? __ldg(xb + k + 1) : 0.0f;
+                            const bool right = rgt > lft;
+                            S += right ? rgt : lft;
+                            j += right ? 1 : 0;
+                        }
+                    }
                 }
                 if (valid) e.level(l, S, plane0, N);
                 else e.reduce(l, S);
@@ -79,7 +98,7 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
     }
 }
 
-template <int L, int OUT>
+template <int VARIANT, int L, int OUT>
 int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     const int N = (int)p->nbins;
@@ -89,7 +108,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
         const int64_t nb = (batch - b0 < max_spectra) ? batch - b0 : max_spectra;
         const int64_t off = b0 * (int64_t)N;
         const dim3 grid((unsigned)tiles, (unsigned)(nb < kGridY ? nb : kGridY), 1);
-        hs_greedy_gather_kernel<L, OUT><<<grid, kThreads, 0, stream>>>(
+        hs_greedy_gather_kernel<VARIANT, L, OUT><<<grid, kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
             buf.amax ? buf.amax + off : nullptr, N, (int)nb);
         HS_CUDA_OK(cudaGetLastError());
@@ -97,28 +116,36 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
     return HS_OK;
 }
 
-template <int L>
+template <int VARIANT, int L>
 int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     switch (p->out_mode) {
-        case HS_OUT_FULL: return launch<L, HS_OUT_FULL>(p, buf, batch, stream);
-        case HS_OUT_REDUCED: return launch<L, HS_OUT_REDUCED>(p, buf, batch, stream);
-        default: return launch<L, HS_OUT_BOTH>(p, buf, batch, stream);
+        case HS_OUT_FULL: return launch<VARIANT, L, HS_OUT_FULL>(p, buf, batch, stream);
+        case HS_OUT_REDUCED: return launch<VARIANT, L, HS_OUT_REDUCED>(p, buf, batch, stream);
+        default: return launch<VARIANT, L, HS_OUT_BOTH>(p, buf, batch, stream);
     }
 }
 
 }  // namespace
 
-int hs_greedy_gather_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+template <int VARIANT>
+static int by_level(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     switch (p->L) {
-        case 1: return by_out<1>(p, buf, batch, stream);
-        case 2: return by_out<2>(p, buf, batch, stream);
-        case 3: return by_out<3>(p, buf, batch, stream);
-        case 4: return by_out<4>(p, buf, batch, stream);
-        case 5: return by_out<5>(p, buf, batch, stream);
-        default: return by_out<6>(p, buf, batch, stream);
+        case 1: return by_out<VARIANT, 1>(p, buf, batch, stream);
+        case 2: return by_out<VARIANT, 2>(p, buf, batch, stream);
+        case 3: return by_out<VARIANT, 3>(p, buf, batch, stream);
+        case 4: return by_out<VARIANT, 4>(p, buf, batch, stream);
+        case 5: return by_out<VARIANT, 5>(p, buf, batch, stream);
+        default: return by_out<VARIANT, 6>(p, buf, batch, stream);
     }
+}
+
+// Greedy (eq. 4) always; freq-bin (eq. 3) as the workspace-free alternative to the two-phase kernel.
+int hs_greedy_gather_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+{
+    if (p->variant == HS_FREQBIN) return by_level<HS_FREQBIN>(p, buf, batch, stream);
+    return by_level<HS_GREEDY>(p, buf, batch, stream);
 }
 
 int hs_greedy_gather_launches(const hs_plan *p, int64_t batch)

@@ -3,9 +3,12 @@
 #include "hs_internal.cuh"
 
 namespace {
-bool two_phase(const hs_plan *p) { return p->variant == HS_FREQBIN || p->variant == HS_MAX; }
+// Max always runs two-phase; freq-bin runs two-phase only when asked to (HS_ALGO_TWOPHASE), else the gather kernel.
+bool two_phase(const hs_plan *p)
+{
+    return p->variant == HS_MAX || (p->variant == HS_FREQBIN && p->algo_req == HS_ALGO_TWOPHASE);
+}
 }  // namespace
-
 bool hs_tiled_supported(const hs_plan *p) { return !two_phase(p) || hs_twophase_supported(p, p->batch); }
 
 size_t hs_tiled_workspace_bytes(const hs_plan *p, int64_t batch)

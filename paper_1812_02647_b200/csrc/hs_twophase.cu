@@ -69,6 +69,7 @@ struct tp_params {
     int ntiles;      // phase-2 items per spectrum
     int D;           // phase 2 lags phase 1 by D spectra
     int R;           // ring slots
+    int discard;     // drop consumed A lines from L2 without write-back
 };
 
 constexpr int chain_len(int j, int hmax)  // K_j: largest power of two with j*K <= hmax
@@ -137,58 +138,78 @@ __device__ __forceinline__ void decimate_chunk(const tp_params &p, const float *
 }
 
 // Max: block maxima of every size 2..HMAX for the super-blocks that start inside the chunk.
+// Odd J >= 3: thread `slot` reduces sub-blocks slot, slot + 256, .. (lane stride J words: conflict-free); all shared
+// and global addresses are base + immediate.  The pyramid pairs neighbouring lanes: sub-block index == lane (mod K).
+template <int J, int HMAX>
+__device__ __forceinline__ void blockmax_j(const tp_params &p, const float *sm, float *Ab, int k0, int lane, int slot)
+{
+    constexpr int K = chain_len(J, HMAX);
+    constexpr int SBW = J * K;                                               // super-block width in words
+    constexpr int U = (((kChunk + SBW - 1) / SBW + 1) * K + kThreads - 1) / kThreads;
+    const int sb_lo = (k0 + SBW - 1) / SBW;                                  // super-blocks that start inside the chunk
+    const int count = ((k0 + kChunk + SBW - 1) / SBW - sb_lo) * K;           // sub-blocks of size J owned by the chunk
+    const int nb = K * sb_lo + slot;                                         // this thread's first sub-block
+    const float *__restrict__ s = sm + (nb * J - k0);
+    float *g[6];                                                             // g[a]: A_{J 2^a} + (nb >> a)
+#pragma unroll
+    for (int a = 0; (1 << a) <= K; a++) g[a] = Ab + p.lay.off[J << a] + (nb >> a);
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const int t = slot + u * kThreads;
+        if ((t & ~31) >= count) break;                                       // warp-uniform: nothing left for this warp
+        const bool live = t < count;
+        const int n = nb + u * kThreads;
+        float v = -INFINITY;
+        if (live) {
+            v = s[u * kThreads * J];
+#pragma unroll
+            for (int w = 1; w < J; w++) v = fmaxf(v, s[u * kThreads * J + w]);
+            if (n < p.lay.len[J]) g[0][u * kThreads] = v;
+        }
+#pragma unroll
+        for (int a = 1; (1 << a) <= K; a++) {                                // blocks of size J 2^a
+            v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1 << (a - 1)));
+            if (live && (lane & ((1 << a) - 1)) == 0 && (n >> a) < p.lay.len[J << a]) g[a][(u * kThreads) >> a] = v;
+        }
+    }
+}
+
+template <int HMAX, int J = 3>
+__device__ __forceinline__ void blockmax_odd(const tp_params &p, const float *sm, float *Ab, int k0, int lane)
+{
+    if constexpr (J <= HMAX) {
+        // rotate the thread -> sub-block assignment by whole warps so that short harmonics do not always load warp 0
+        const int slot = (threadIdx.x + 32 * ((J >> 1) & (kWarps - 1))) & (kThreads - 1);
+        blockmax_j<J, HMAX>(p, sm, Ab, k0, lane, slot);
+        blockmax_odd<HMAX, J + 2>(p, sm, Ab, k0, lane);
+    }
+}
+
 template <int HMAX>
 __device__ __forceinline__ void blockmax_chunk(const tp_params &p, const float *sm, float *Ab, int k0)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // ---- j = 1 chain (sizes 2,4,..,HMAX): one aligned float4 per thread, then a shuffle pyramid -------------------
+    const int lane = threadIdx.x & 31;
+    // ---- J = 1 chain (sizes 2,4,..,HMAX): one aligned float4 per thread, then a shuffle pyramid -------------------
     if (HMAX >= 2) {
+        float *g[6];                                                         // g[a]: A_{2^a} + ((k0 + 4 tid) >> a)
+#pragma unroll
+        for (int a = 1; (1 << a) <= HMAX; a++) g[a] = Ab + p.lay.off[1 << a] + ((k0 + 4 * threadIdx.x) >> a);
 #pragma unroll
         for (int r = 0; r < kChunk / (4 * kThreads); r++) {
-            const int q = r * kThreads + threadIdx.x;              // float4 index inside the chunk (k0 % 32 == 0)
-            const int k = k0 + 4 * q;
-            const float4 v = reinterpret_cast<const float4 *>(sm)[q];
+            const int k = k0 + 4 * (r * kThreads + threadIdx.x);           // k0 % 4096 == 0: k / 4 == lane (mod 32)
+            const float4 v = reinterpret_cast<const float4 *>(sm)[r * kThreads + threadIdx.x];
             const float m2a = fmaxf(v.x, v.y), m2b = fmaxf(v.z, v.w);
-            if (k < 2 * p.lay.len[2]) *reinterpret_cast<float2 *>(Ab + p.lay.off[2] + (k >> 1)) = make_float2(m2a, m2b);
+            if (k < 2 * p.lay.len[2]) *reinterpret_cast<float2 *>(g[1] + ((4 * r * kThreads) >> 1)) = make_float2(m2a, m2b);
             float m = fmaxf(m2a, m2b);
-            if (HMAX >= 4 && k < 4 * p.lay.len[4]) Ab[p.lay.off[4] + (k >> 2)] = m;
+            if (HMAX >= 4 && k < 4 * p.lay.len[4]) g[2][(4 * r * kThreads) >> 2] = m;
 #pragma unroll
-            for (int a = 3; (1 << a) <= HMAX; a++) {                // sizes 8, 16, 32: pairs of lanes
+            for (int a = 3; (1 << a) <= HMAX; a++) {                        // sizes 8, 16, 32: pairs of lanes
                 m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1 << (a - 3)));
-                if ((lane & ((1 << (a - 2)) - 1)) == 0 && (k >> a) < p.lay.len[1 << a]) Ab[p.lay.off[1 << a] + (k >> a)] = m;
+                if ((lane & ((1 << (a - 2)) - 1)) == 0 && (k >> a) < p.lay.len[1 << a]) g[a][(4 * r * kThreads) >> a] = m;
             }
         }
     }
-    // ---- odd j >= 3 -------------------------------------------------------------------------------------------------
-    int task0 = 0;  // running count of warp-tasks handed out so far (mod kWarps): spreads the harmonics over the warps
-#pragma unroll
-    for (int j = 3; j <= HMAX; j += 2) {
-        const int K = chain_len(j, HMAX);
-        const int sbw = j * K;                                  // super-block width in words
-        const int sb_lo = (k0 + sbw - 1) / sbw;                 // super-blocks that start inside the chunk
-        const int sb_hi = (k0 + kChunk + sbw - 1) / sbw;
-        const int count = (sb_hi - sb_lo) * K;                  // sub-blocks of size j; the first is K*sb_lo
-        const int ntask = (count + 31) >> 5;                    // one warp-task = 32 consecutive sub-blocks
-        const int first = (warp - task0) & (kWarps - 1);
-        for (int tk = first; tk < ntask; tk += kWarps) {
-            const int t = tk * 32 + lane;
-            const bool live = t < count;
-            const int n = K * sb_lo + (live ? t : 0);            // sub-block index; n == lane (mod K)
-            const float *__restrict__ s = sm + (n * j - k0);
-            float v = s[0];
-#pragma unroll
-            for (int u = 1; u < j; u++) v = fmaxf(v, s[u]);
-            if (live && n < p.lay.len[j]) Ab[p.lay.off[j] + n] = v;
-#pragma unroll
-            for (int a = 1; (1 << a) <= K; a++) {               // pyramid: blocks of size j*2^a
-                v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1 << (a - 1)));
-                const int i = j << a;
-                const int na = n >> a;
-                if (live && (lane & ((1 << a) - 1)) == 0 && na < p.lay.len[i]) Ab[p.lay.off[i] + na] = v;
-            }
-        }
-        task0 = (task0 + ntask) & (kWarps - 1);
-    }
+    blockmax_odd<HMAX>(p, sm, Ab, k0, lane);
 }
 
 // ---------------------------------------------------------------------------------------------- phase 2
@@ -199,6 +220,7 @@ __device__ __forceinline__ void phase2_round(const tp_params &p, const float *__
     const int n_first = n & ~127;                                  // first bin of this warp (warp = 128 bins)
     hs_emit<OUT> e0, e1, e2, e3;
     float *plane0 = (OUT & HS_OUT_FULL) ? p.sums + row * L + n : nullptr;
+    const float *__restrict__ An = Ab + n;                         // A_i[n] = An[off_i]
     auto emit = [&](int l) {
         const float4 h = make_float4(S.x * hs_norm(l), S.y * hs_norm(l), S.z * hs_norm(l), S.w * hs_norm(l));
         if (OUT & HS_OUT_FULL) hsptx::st_cs(reinterpret_cast<float4 *>(plane0 + (int64_t)l * N), h);
@@ -218,18 +240,22 @@ __device__ __forceinline__ void phase2_round(const tp_params &p, const float *__
             if (hi * (n_first + 128) <= N) {                       // warp-uniform: every element of the level in range
 #pragma unroll
                 for (int i = lo; i <= hi; i++) {
-                    const float4 v = hsptx::ld_cg(reinterpret_cast<const float4 *>(Ab + p.lay.off[i] + n));
+                    const float4 v = hsptx::ld_cg(reinterpret_cast<const float4 *>(An + p.lay.off[i]));
                     S.x += v.x;
                     S.y += v.y;
                     S.z += v.z;
                     S.w += v.w;
+                    // This 128-byte line of A_i is read by exactly these 8 lanes and never again: drop it from L2 so
+                    // that the dead data is not written back to HBM.  The test on v.x makes the discard wait for the load.
+                    if (p.discard && (threadIdx.x & 7) == 0 && v.x == v.x)
+                        asm volatile("discard.global.L2 [%0], 128;" ::"l"(An + p.lay.off[i]) : "memory");
                 }
             } else {
 #pragma unroll
                 for (int i = lo; i <= hi; i++) {
                     const int len = p.lay.len[i];
                     if (n < len) {
-                        const float4 v = hsptx::ld_cg(reinterpret_cast<const float4 *>(Ab + p.lay.off[i] + n));
+                        const float4 v = hsptx::ld_cg(reinterpret_cast<const float4 *>(An + p.lay.off[i]));
                         S.x += v.x;                               // n < len
                         S.y += (n + 1 < len) ? v.y : 0.f;
                         S.z += (n + 2 < len) ? v.z : 0.f;
@@ -430,6 +456,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.ntiles = s.ntiles;
     prm.D = s.D;
     prm.R = s.R;
+    prm.discard = tune_int("HS_TP_DISCARD", 0);
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(batch), stream));
     const int64_t total = (int64_t)(batch + s.D) * (s.nchunks + s.ntiles);
     const unsigned grid = (unsigned)(total < s.grid ? total : s.grid);

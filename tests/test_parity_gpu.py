@@ -15,7 +15,7 @@ from parity import argmax_from_levels, check_argmax, check_sums
 pytestmark = pytest.mark.gpu
 
 VARIANTS = ["standard", "max", "freqbin", "greedy"]
-ALGOS = ["direct", "tiled"]
+ALGOS = ["direct", "tiled", "twophase"]
 
 
 @pytest.fixture(scope="module")
@@ -30,9 +30,11 @@ def hs():
 
 def make_plan(hs, N, B, Hmax, variant, out_mode, algo):
     plan = hs.hs_plan_create(N, B, Hmax, variant, out_mode)
-    if algo == "tiled":
+    if algo in ("tiled", "twophase"):
+        if algo == "twophase" and variant != "freqbin":
+            pytest.skip("two-phase is a separate choice for freq-bin only (Max: same as tiled)")
         try:
-            plan.set_algo("tiled")
+            plan.set_algo(algo)
         except hs.HsError:
             pytest.skip("no tuned kernel covers this plan")
     else:
@@ -226,6 +228,8 @@ def test_error_paths_on_device(hs):
     assert plan.launches() >= 1 and plan.levels == 6
     with pytest.raises(hs.HsError):
         plan.set_algo(7)
+    with pytest.raises(hs.HsError):
+        g.set_algo("twophase")            # eq. 1 has no two-phase kernel
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
