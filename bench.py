@@ -274,6 +274,12 @@ def main():
                           "bins_per_s": batch * nbins / (per_variant_ms[v] * 1e-3), "eff_GBps": gbs,
                           "frac_of_measured_peak": gbs / peak, "frac_of_nominal_8TBps": gbs / 8000.0,
                           "algo": algo_names[plans[v].algo], "launches": plans[v].launches()}
+        ws = plans[v]._ws
+        if ws is not None and ws.numel() >= 64 and v in ("max", "freqbin"):
+            # two-phase kernel's dependency-wait statistics (workspace words 2..5, see hs_twophase.cu)
+            c = ws[:64].view(torch.int32).cpu().tolist()
+            per_variant[v]["waits"] = {"ring_waits": c[2], "ring_spins": c[3], "phase2_waits": c[4], "phase2_spins": c[5],
+                                       "workspace_MiB": round(plans[v].workspace_bytes() / 2**20)}
     dominant = max(variants, key=lambda v: per_variant_ms[v])
     dom_algo = per_variant[dominant]["algo"]
     roofline = {"bound": "hbm", "kernel": f"{dominant} ({dom_algo})", "achieved": per_variant[dominant]["eff_GBps"],

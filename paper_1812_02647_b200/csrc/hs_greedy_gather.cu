@@ -13,13 +13,17 @@
 namespace {
 
 constexpr int kThreads = 128;
-constexpr int kGridY = 32;   // spectra are strided over gridDim.y so that the per-thread prologue is amortised
+constexpr int kSpectraPerCta = 8;  // spectra run side by side per thread (tuned on B200: 2 -> 5.6 ms, 4 -> 4.9, 8 -> 4.7, 16 -> 5.4 for eq. 3)
+constexpr int kGridY = 65535; // blockIdx.y = spectrum: CTAs are dispatched x-fastest, i.e. spectrum-major, so the gathers of
+                              // all harmonics of one spectrum (1 MiB) happen close in time and hit L2 (ncu: 4 B/bin of DRAM
+                              // reads; striding spectra over a small gridDim.y instead thrashed L2 at 28-33 B/bin)
 
 template <int VARIANT, int L, int OUT>
-__global__ void __launch_bounds__(kThreads, 12)
+__global__ void __launch_bounds__(kThreads, 8)
 hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
                         uint8_t *__restrict__ amax, int N, int batch)
 {
+    constexpr int Q = kSpectraPerCta;
     const int n = blockIdx.x * kThreads + threadIdx.x;
     const int n_lo = n & ~31;                      // first bin of this warp
     if (n_lo >= N) return;
@@ -28,14 +32,45 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
     const int n_hi1 = min(n_lo + 32, N);           // one past the warp's last bin
     // Warp-uniform range tests (no divisions): harmonic i is in range for EVERY lane, neighbour included, iff
     // i * n_hi1 <= N; it is in range for SOME lane iff i * n_lo < N.
-    for (int b = blockIdx.y; b < batch; b += gridDim.y) {
-        const float *__restrict__ xb = x + b * (int64_t)N;
-        hs_emit<OUT> e;
-        float *plane0 = (OUT & HS_OUT_FULL) ? sums + ((int64_t)b * L) * N + nn : nullptr;
-        float S = __ldg(xb + nn);
-        if (valid) e.level(0, S, plane0, N);
-        else e.reduce(0, S);
-        int j = 0;
+    // A thread runs the same bin of Q consecutive spectra side by side: the control flow depends on n only, so the Q
+    // chains share every bound and give Q independent loads in flight (Greedy's chain is serial within a spectrum).
+    for (int b0 = blockIdx.y * Q; b0 < batch; b0 += gridDim.y * Q) {
+        const float *__restrict__ xb[Q];
+        bool live[Q];
+        hs_emit<OUT> e[Q];
+        float S[Q];
+        int j[Q];
+#pragma unroll
+        for (int q = 0; q < Q; q++) {
+            live[q] = valid && b0 + q < batch;
+            xb[q] = x + (int64_t)min(b0 + q, batch - 1) * N;          // spectra past the batch shadow the last one
+            S[q] = __ldg(xb[q] + nn);
+            j[q] = 0;
+        }
+        auto emit = [&](int l) {
+#pragma unroll
+            for (int q = 0; q < Q; q++) {
+                const float h = S[q] * hs_norm(l);
+                if ((OUT & HS_OUT_FULL) && live[q]) hsptx::st_cs(sums + (((int64_t)(b0 + q) * L + l) * N + nn), h);
+                if (OUT & HS_OUT_REDUCED) e[q].reduce(l, h);
+            }
+        };
+        auto step = [&](int base, bool safe) {      // harmonic with i * n == base
+#pragma unroll
+            for (int q = 0; q < Q; q++) {
+                if (VARIANT == HS_FREQBIN) {        // eq. 3: x~(i n)
+                    S[q] += (safe || base < N) ? __ldg(xb[q] + base) : 0.0f;
+                } else {                            // eq. 4: max of the bin under the drift and its right neighbour
+                    const int k = base + j[q];
+                    const float lft = (safe || k < N) ? __ldg(xb[q] + k) : 0.0f;
+                    const float rgt = (safe || k + 1 < N) ? __ldg(xb[q] + k + 1) : 0.0f;
+                    const bool right = rgt > lft;   // strictly greater (C4)
+                    S[q] += right ? rgt : lft;
+                    j[q] += right ? 1 : 0;
+                }
+            }
+        };
+        emit(0);
         bool tail = false;
 #pragma unroll
         for (int l = 1; l < L; l++) {
@@ -43,57 +78,32 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
             if (lo * n_lo < N) {                    // some harmonic of this level is in range for some lane
                 int i = lo;
                 int base = (lo - 1) * nn;           // (i - 1) * n
-                if (VARIANT == HS_FREQBIN && hi * n_hi1 <= N) {   // whole level in range for every lane: fixed trip count
-                    {    // eq. 3: x(i n); the loads are independent and all in flight at once
-                        float v[16];
-#pragma unroll
-                        for (int q = 0; q < 16; q++)
-                            if (q <= hi - lo) v[q] = __ldg(xb + (lo + q) * nn);
-#pragma unroll
-                        for (int q = 0; q < 16; q++)
-                            if (q <= hi - lo) S += v[q];
-                    }
-                } else {
-                    for (; i <= hi && i * n_hi1 <= N; i++) {
-                        base += nn;
-                        if (VARIANT == HS_FREQBIN) {
-                            S += __ldg(xb + base);
-                        } else {
-                            const float *__restrict__ p = xb + (base + j);
-                            const float lft = __ldg(p), rgt = __ldg(p + 1);
-                            const bool right = rgt > lft;
-                            S += right ? rgt : lft;
-                            j += right ? 1 : 0;
-                        }
-                    }
-                    for (; i <= hi && i * n_lo < N; i++) {
-                        base += nn;
-                        if (VARIANT == HS_FREQBIN) {
-                            S += base < N ? __ldg(xb + base) : 0.0f;
-                        } else {
-                            const int k = base + j;
-                            const float lft = k < N ? __ldg(xb + k) : 0.0f;
-                            const float rgt = k + 1 < N ? __ldg(xb + k + 1) : 0.0f;
-                            const bool right = rgt > lft;
-                            S += right ? rgt : lft;
-                            j += right ? 1 : 0;
-                        }
-                    }
+                for (; i <= hi && i * n_hi1 <= N; i++) {
+                    base += nn;
+                    step(base, true);
                 }
-                if (valid) e.level(l, S, plane0, N);
-                else e.reduce(l, S);
+                for (; i <= hi && i * n_lo < N; i++) {
+                    base += nn;
+                    step(base, false);
+                }
+                emit(l);
             } else if (OUT != HS_OUT_REDUCED) {
-                if (valid) e.level(l, S, plane0, N);
+                emit(l);
             } else {
                 tail = true;
             }
         }
         // Levels whose harmonics are all out of range leave S unchanged, and h_l = S c_l is monotone in l: for S >= 0
         // no later level exceeds the running maximum, for S < 0 the last level is the largest.  Test level L-1 only.
-        if (OUT == HS_OUT_REDUCED && tail) e.reduce(L - 1, S * hs_norm(L - 1));
-        if ((OUT & HS_OUT_REDUCED) && valid) {
-            hsptx::st_cs(vmax + b * (int64_t)N + n, e.m);
-            hsptx::st_cs(amax + b * (int64_t)N + n, (uint8_t)e.a);
+        if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
+        if (OUT & HS_OUT_REDUCED) {
+#pragma unroll
+            for (int q = 0; q < Q; q++) {
+                if (live[q]) {
+                    hsptx::st_cs(vmax + (int64_t)(b0 + q) * N + n, e[q].m);
+                    hsptx::st_cs(amax + (int64_t)(b0 + q) * N + n, (uint8_t)e[q].a);
+                }
+            }
         }
     }
 }
@@ -107,7 +117,8 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
     for (int64_t b0 = 0; b0 < batch; b0 += max_spectra) {
         const int64_t nb = (batch - b0 < max_spectra) ? batch - b0 : max_spectra;
         const int64_t off = b0 * (int64_t)N;
-        const dim3 grid((unsigned)tiles, (unsigned)(nb < kGridY ? nb : kGridY), 1);
+        const int64_t gy = (nb + kSpectraPerCta - 1) / kSpectraPerCta;
+        const dim3 grid((unsigned)tiles, (unsigned)(gy < kGridY ? gy : kGridY), 1);
         hs_greedy_gather_kernel<VARIANT, L, OUT><<<grid, kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
             buf.amax ? buf.amax + off : nullptr, N, (int)nb);

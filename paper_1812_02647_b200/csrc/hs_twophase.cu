@@ -424,11 +424,16 @@ tp_sched make_sched(const hs_plan *p, int64_t batch)
     const int per_round = s.nchunks + s.ntiles;
     // lag: enough rounds that the CTAs in flight never reach a phase-2 item before its phase-1 items have finished
     (void)per_round;
-    const int in_flight = s.nchunks > 0 ? (s.grid + s.nchunks - 1) / s.nchunks : 0;   // rounds of phase-1 items in flight
-    int D = tune_int("HS_TP_LAG", in_flight + 2);
+    // Items are claimed in order but finish out of order: a CTA holds up to three claimed items (running, preloaded,
+    // prefetched index), and a phase-2 item that has to spin delays the phase-1 items queued behind it in the same CTA,
+    // which in turn makes later phase-2 items spin (a convoy).  Measured on B200 (profiles/r01_twophase_lag.md): with
+    // 4 CTAs/SM the spinning only vanishes once phase 2 lags by about six times the items in flight, and the ring
+    // needs as much slack again.  That is ~0.8 GB of workspace whatever the spectrum length; it no longer fits L2.
+    const int in_flight = s.nchunks > 0 ? (6 * s.grid + s.nchunks - 1) / s.nchunks : 0;
+    int D = tune_int("HS_TP_LAG", in_flight + 1);
     if (D > batch) D = (int)batch;
     if (D < 1) D = 1;
-    int R = tune_int("HS_TP_RING", 2 * D);
+    int R = tune_int("HS_TP_RING", 4 * D);
     if (R > batch) R = (int)batch;
     if (R < D) R = D;          // (R >= D keeps slot b-R's phase 2 strictly before phase 1 of b in the item order)
     s.D = D;
