@@ -137,79 +137,88 @@ __device__ __forceinline__ void decimate_chunk(const tp_params &p, const float *
     }
 }
 
-// Max: block maxima of every size 2..HMAX for the super-blocks that start inside the chunk.
-// Odd J >= 3: thread `slot` reduces sub-blocks slot, slot + 256, .. (lane stride J words: conflict-free); all shared
-// and global addresses are base + immediate.  The pyramid pairs neighbouring lanes: sub-block index == lane (mod K).
-template <int J, int HMAX>
-__device__ __forceinline__ void blockmax_j(const tp_params &p, const float *sm, float *Ab, int k0, int lane, int slot)
+// Max: A_i[n] = max x~[i n .. i n + i - 1] for the blocks that start inside the chunk, via sliding-maximum tables
+// (a two-level sparse table): T4[x] = max w[x..x+3] and T16[x] = max w[x..x+15] are built IN PLACE in the chunk's
+// shared-memory buffer (float4 per thread: read, barrier, write, barrier), and a block of size i is the maximum of
+// ceil(i / TW) table entries: offsets 0, TW, 2 TW, .. and i - TW (overlapping reads are harmless for a maximum).
+// That is 2-4 shared-memory reads per block instead of i, and the same base + immediate addressing as decimate_one.
+template <int I, int TW>
+__device__ __forceinline__ void blockmax_query(const float *s_base /* sm - k0 */, float *__restrict__ Ai, int2 bd)
 {
-    constexpr int K = chain_len(J, HMAX);
-    constexpr int SBW = J * K;                                               // super-block width in words
-    constexpr int U = (((kChunk + SBW - 1) / SBW + 1) * K + kThreads - 1) / kThreads;
-    const int sb_lo = (k0 + SBW - 1) / SBW;                                  // super-blocks that start inside the chunk
-    const int count = ((k0 + kChunk + SBW - 1) / SBW - sb_lo) * K;           // sub-blocks of size J owned by the chunk
-    const int nb = K * sb_lo + slot;                                         // this thread's first sub-block
-    const float *__restrict__ s = sm + (nb * J - k0);
-    float *g[6];                                                             // g[a]: A_{J 2^a} + (nb >> a)
+    constexpr int TMAX = (kChunk / I + 1 + kThreads - 1) / kThreads;
+    const int n0 = bd.x + threadIdx.x;
+    const float *__restrict__ s = s_base + I * n0;
+    float *__restrict__ g = Ai + n0;
 #pragma unroll
-    for (int a = 0; (1 << a) <= K; a++) g[a] = Ab + p.lay.off[J << a] + (nb >> a);
+    for (int t = 0; t < TMAX; t++) {
+        if (n0 + t * kThreads < bd.y) {
+            float v = s[I * t * kThreads];
 #pragma unroll
-    for (int u = 0; u < U; u++) {
-        const int t = slot + u * kThreads;
-        if ((t & ~31) >= count) break;                                       // warp-uniform: nothing left for this warp
-        const bool live = t < count;
-        const int n = nb + u * kThreads;
-        float v = -INFINITY;
-        if (live) {
-            v = s[u * kThreads * J];
-#pragma unroll
-            for (int w = 1; w < J; w++) v = fmaxf(v, s[u * kThreads * J + w]);
-            if (n < p.lay.len[J]) g[0][u * kThreads] = v;
-        }
-#pragma unroll
-        for (int a = 1; (1 << a) <= K; a++) {                                // blocks of size J 2^a
-            v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1 << (a - 1)));
-            if (live && (lane & ((1 << a) - 1)) == 0 && (n >> a) < p.lay.len[J << a]) g[a][(u * kThreads) >> a] = v;
+            for (int o = TW; o + TW < I; o += TW) v = fmaxf(v, s[I * t * kThreads + o]);
+            if (I > TW) v = fmaxf(v, s[I * t * kThreads + I - TW]);
+            g[t * kThreads] = v;
         }
     }
 }
 
-template <int HMAX, int J = 3>
-__device__ __forceinline__ void blockmax_odd(const tp_params &p, const float *sm, float *Ab, int k0, int lane)
+template <int HMAX, int TW, int I, int IEND>
+__device__ __forceinline__ void blockmax_range(const tp_params &p, const float *s_base, const int2 *bounds, float *Ab)
 {
-    if constexpr (J <= HMAX) {
-        // rotate the thread -> sub-block assignment by whole warps so that short harmonics do not always load warp 0
-        const int slot = (threadIdx.x + 32 * ((J >> 1) & (kWarps - 1))) & (kThreads - 1);
-        blockmax_j<J, HMAX>(p, sm, Ab, k0, lane, slot);
-        blockmax_odd<HMAX, J + 2>(p, sm, Ab, k0, lane);
+    if constexpr (I <= IEND && I <= HMAX) {
+        blockmax_query<I, TW>(s_base, Ab + p.lay.off[I], bounds[I]);
+        blockmax_range<HMAX, TW, I + 1, IEND>(p, s_base, bounds, Ab);
     }
 }
 
-template <int HMAX>
-__device__ __forceinline__ void blockmax_chunk(const tp_params &p, const float *sm, float *Ab, int k0)
+constexpr int kGroups = (kChunk + kHalo) / 4;                       // float4 groups holding real data
+constexpr int kBuildRounds = (kGroups + kThreads - 1) / kThreads;
+
+// T_{4 w}[x] = max(T_w[x], T_w[x+w], T_w[x+2w], T_w[x+3w]) in place; W4 = w / 4 in float4 groups, or 0 for the first
+// level (raw words -> T4, unaligned neighbours).
+template <int W4>
+__device__ __forceinline__ void build_table(float *sm)
 {
-    const int lane = threadIdx.x & 31;
-    // ---- J = 1 chain (sizes 2,4,..,HMAX): one aligned float4 per thread, then a shuffle pyramid -------------------
-    if (HMAX >= 2) {
-        float *g[6];                                                         // g[a]: A_{2^a} + ((k0 + 4 tid) >> a)
+    float4 *sm4 = reinterpret_cast<float4 *>(sm);
+    float4 r[kBuildRounds];
 #pragma unroll
-        for (int a = 1; (1 << a) <= HMAX; a++) g[a] = Ab + p.lay.off[1 << a] + ((k0 + 4 * threadIdx.x) >> a);
-#pragma unroll
-        for (int r = 0; r < kChunk / (4 * kThreads); r++) {
-            const int k = k0 + 4 * (r * kThreads + threadIdx.x);           // k0 % 4096 == 0: k / 4 == lane (mod 32)
-            const float4 v = reinterpret_cast<const float4 *>(sm)[r * kThreads + threadIdx.x];
-            const float m2a = fmaxf(v.x, v.y), m2b = fmaxf(v.z, v.w);
-            if (k < 2 * p.lay.len[2]) *reinterpret_cast<float2 *>(g[1] + ((4 * r * kThreads) >> 1)) = make_float2(m2a, m2b);
-            float m = fmaxf(m2a, m2b);
-            if (HMAX >= 4 && k < 4 * p.lay.len[4]) g[2][(4 * r * kThreads) >> 2] = m;
-#pragma unroll
-            for (int a = 3; (1 << a) <= HMAX; a++) {                        // sizes 8, 16, 32: pairs of lanes
-                m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1 << (a - 3)));
-                if ((lane & ((1 << (a - 2)) - 1)) == 0 && (k >> a) < p.lay.len[1 << a]) g[a][(4 * r * kThreads) >> a] = m;
+    for (int q = 0; q < kBuildRounds; q++) {
+        const int g = q * kThreads + threadIdx.x;
+        if (g < kGroups) {
+            if (W4 == 0) {
+                const float4 a = sm4[g], b = sm4[g + 1];
+                const float m12 = fmaxf(a.y, a.z), m23 = fmaxf(a.z, a.w), m30 = fmaxf(a.w, b.x);
+                r[q] = make_float4(fmaxf(fmaxf(a.x, a.y), m23), fmaxf(m12, m30), fmaxf(m23, fmaxf(b.x, b.y)),
+                                   fmaxf(m30, fmaxf(b.y, b.z)));
+            } else {
+                const float4 a = sm4[g], b = sm4[g + W4], c = sm4[g + 2 * W4], d = sm4[g + 3 * W4];
+                r[q] = make_float4(fmaxf(fmaxf(a.x, b.x), fmaxf(c.x, d.x)), fmaxf(fmaxf(a.y, b.y), fmaxf(c.y, d.y)),
+                                   fmaxf(fmaxf(a.z, b.z), fmaxf(c.z, d.z)), fmaxf(fmaxf(a.w, b.w), fmaxf(c.w, d.w)));
             }
         }
     }
-    blockmax_odd<HMAX>(p, sm, Ab, k0, lane);
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < kBuildRounds; q++) {
+        const int g = q * kThreads + threadIdx.x;
+        if (g < kGroups) sm4[g] = r[q];
+    }
+    __syncthreads();
+}
+
+template <int HMAX>
+__device__ __forceinline__ void blockmax_chunk(const tp_params &p, float *sm, const int2 *bounds, float *Ab, int k0)
+{
+    const float *s_base = sm - k0;
+    blockmax_range<HMAX, 1, 2, 3>(p, s_base, bounds, Ab);           // sizes 2, 3 from the raw words
+    if (HMAX >= 4) {
+        build_table<0>(sm);                                         // T4
+        blockmax_range<HMAX, 4, 4, 15>(p, s_base, bounds, Ab);
+        if (HMAX == 16) blockmax_range<HMAX, 4, 16, 16>(p, s_base, bounds, Ab);
+    }
+    if (HMAX >= 32) {
+        build_table<1>(sm);                                         // T16
+        blockmax_range<HMAX, 16, 16, 32>(p, s_base, bounds, Ab);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------- phase 2
@@ -327,7 +336,7 @@ tp_persistent_kernel(const __grid_constant__ tp_params p)
 {
     static_assert(kChunk == kTile2, "preload() addresses both phases the same way");
     constexpr int L = HMAX == 1 ? 1 : HMAX == 2 ? 2 : HMAX == 4 ? 3 : HMAX == 8 ? 4 : HMAX == 16 ? 5 : 6;
-    __shared__ __align__(16) float sm[kChunk + kHalo];
+    __shared__ __align__(16) float sm[kChunk + kHalo + 16];        // + zero pad read by the table builds
     __shared__ int2 s_bounds[33];
     __shared__ int s_item[2];
     int *queue = p.ctrl, *err = p.ctrl + 1;
@@ -335,6 +344,7 @@ tp_persistent_kernel(const __grid_constant__ tp_params p)
     const int64_t total = (int64_t)(p.B + p.D) * (p.nchunks + p.ntiles);
     const int N = p.N;
 
+    if (threadIdx.x < 16) sm[kChunk + kHalo + threadIdx.x] = 0.0f;
     if (threadIdx.x == 0) {
         s_item[0] = atomicAdd(queue, 1);
         s_item[1] = atomicAdd(queue, 1);
@@ -356,7 +366,7 @@ tp_persistent_kernel(const __grid_constant__ tp_params p)
             for (int q = 0; q < kChunk / (4 * kThreads); q++)
                 reinterpret_cast<float4 *>(sm)[q * kThreads + threadIdx.x] = pre.v[q];
             if (threadIdx.x < kHalo / 4) reinterpret_cast<float4 *>(sm)[kChunk / 4 + threadIdx.x] = pre.halo;
-            if (VARIANT == HS_FREQBIN && threadIdx.x >= 2 && threadIdx.x <= HMAX) {
+            if (threadIdx.x >= 2 && threadIdx.x <= HMAX) {
                 const int i = threadIdx.x;
                 s_bounds[i] = make_int2((k0 + i - 1) / i, min((k0 + kChunk + i - 1) / i, p.lay.len[i]));
             }
@@ -366,7 +376,7 @@ tp_persistent_kernel(const __grid_constant__ tp_params p)
             __syncthreads();
             float *Ab = p.A + (int64_t)(b % p.R) * p.lay.slot_words;
             if (VARIANT == HS_FREQBIN) decimate_chunk<HMAX>(p, sm - k0, s_bounds, Ab);
-            else blockmax_chunk<HMAX>(p, sm, Ab, k0);
+            else blockmax_chunk<HMAX>(p, sm, s_bounds, Ab, k0);
             if (threadIdx.x == 0) s_item[flip] = after;
             __syncthreads();                                         // all stores of the CTA are ordered before ...
             if (threadIdx.x == 0) red_release_add(cnt1 + b, 1);      // ... thread 0's release (cumulative, gpu scope)
@@ -401,6 +411,56 @@ tp_persistent_kernel(const __grid_constant__ tp_params p)
     }
 }
 
+// ---------------------------------------------------------------------------------------------- plain two-launch path
+// The same phase bodies as two ordinary kernels over a group of spectra (one CTA per item, the hardware scheduler
+// instead of the work counter, stream order instead of the dependency counters).  Each kernel has its own register
+// budget, so more CTAs fit per SM than in the fused persistent kernel.
+template <int VARIANT, int HMAX>
+__global__ void __launch_bounds__(kThreads, 6)
+tp_phase1_kernel(const __grid_constant__ tp_params p, int b0)
+{
+    __shared__ __align__(16) float sm[kChunk + kHalo + 16];
+    __shared__ int2 s_bounds[33];
+    const int b = b0 + blockIdx.y, chunk = blockIdx.x;
+    const int k0 = chunk * kChunk, N = p.N;
+    if (threadIdx.x < 16) sm[kChunk + kHalo + threadIdx.x] = 0.0f;
+    tp_pre pre;
+    preload(p, tp_item{1, b, chunk}, pre);
+#pragma unroll
+    for (int q = 0; q < kChunk / (4 * kThreads); q++) reinterpret_cast<float4 *>(sm)[q * kThreads + threadIdx.x] = pre.v[q];
+    if (threadIdx.x < kHalo / 4) reinterpret_cast<float4 *>(sm)[kChunk / 4 + threadIdx.x] = pre.halo;
+    if (threadIdx.x >= 2 && threadIdx.x <= HMAX) {
+        const int i = threadIdx.x;
+        s_bounds[i] = make_int2((k0 + i - 1) / i, min((k0 + kChunk + i - 1) / i, p.lay.len[i]));
+    }
+    __syncthreads();
+    float *Ab = p.A + (int64_t)(b % p.R) * p.lay.slot_words;
+    if (VARIANT == HS_FREQBIN) decimate_chunk<HMAX>(p, sm - k0, s_bounds, Ab);
+    else blockmax_chunk<HMAX>(p, sm, s_bounds, Ab, k0);
+    (void)N;
+}
+
+template <int L, int OUT>
+__global__ void __launch_bounds__(kThreads, 4)
+tp_phase2_kernel(const __grid_constant__ tp_params p, int b0)
+{
+    const int b = b0 + blockIdx.y, N = p.N;
+    const int64_t row = (int64_t)b * N;
+    const int n0 = blockIdx.x * kTile2 + 4 * threadIdx.x;
+    const float *Ab = p.A + (int64_t)(b % p.R) * p.lay.slot_words;
+    float4 S[kRounds2];
+#pragma unroll
+    for (int q = 0; q < kRounds2; q++) {
+        const int n = n0 + q * (4 * kThreads);
+        S[q] = n < N ? __ldg(reinterpret_cast<const float4 *>(p.x + row + n)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+#pragma unroll
+    for (int q = 0; q < kRounds2; q++) {
+        const int n = n0 + q * (4 * kThreads);
+        if (n < N) phase2_round<L, OUT>(p, Ab, row, n, S[q]);
+    }
+}
+
 // tuning knobs for experiments (environment, read when the schedule is built); defaults are the tuned values
 int tune_int(const char *name, int dflt)
 {
@@ -410,6 +470,7 @@ int tune_int(const char *name, int dflt)
 
 struct tp_sched {
     int nchunks, ntiles, D, R, grid;
+    bool plain;
     tp_layout lay;
 };
 
@@ -438,6 +499,18 @@ tp_sched make_sched(const hs_plan *p, int64_t batch)
     if (R < D) R = D;          // (R >= D keeps slot b-R's phase 2 strictly before phase 1 of b in the item order)
     s.D = D;
     s.R = R < 1 ? 1 : R;
+    s.plain = tune_int("HS_TP_MODE", 1) == 1;
+    if (s.plain) {
+        // plain two-launch mode: groups of up to 512 spectra (1.6 GB of A arrays at 2^18 bins); bigger groups mean
+        // fewer, longer kernels (B200: 256 -> 9.8 ms, 512 -> 9.2 ms, 1024 -> 8.6 ms for eq. 2 on 4096 x 2^18)
+        int64_t G = tune_int("HS_TP_RING", 0);
+        if (G <= 0) {
+            G = s.lay.slot_words > 0 ? ((int64_t)1600 << 20) / (s.lay.slot_words * 4) : batch;
+            if (G > 65535) G = 65535;
+        }
+        if (G > batch) G = batch;
+        s.R = G < 1 ? 1 : (int)G;
+    }
     return s;
 }
 
@@ -462,6 +535,20 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.D = s.D;
     prm.R = s.R;
     prm.discard = tune_int("HS_TP_DISCARD", 0);
+    if (s.plain) {
+        // plain path: groups of R spectra, phase 1 then phase 2 in stream order
+        constexpr int L = HMAX == 1 ? 1 : HMAX == 2 ? 2 : HMAX == 4 ? 3 : HMAX == 8 ? 4 : HMAX == 16 ? 5 : 6;
+        for (int64_t b0 = 0; b0 < batch; b0 += s.R) {
+            const int nb = (int)((batch - b0 < s.R) ? batch - b0 : s.R);
+            if (s.nchunks > 0) {
+                tp_phase1_kernel<VARIANT, HMAX><<<dim3((unsigned)s.nchunks, (unsigned)nb), kThreads, 0, stream>>>(prm, (int)b0);
+                HS_CUDA_OK(cudaGetLastError());
+            }
+            tp_phase2_kernel<L, OUT><<<dim3((unsigned)s.ntiles, (unsigned)nb), kThreads, 0, stream>>>(prm, (int)b0);
+            HS_CUDA_OK(cudaGetLastError());
+        }
+        return HS_OK;
+    }
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(batch), stream));
     const int64_t total = (int64_t)(batch + s.D) * (s.nchunks + s.ntiles);
     const unsigned grid = (unsigned)(total < s.grid ? total : s.grid);
@@ -502,7 +589,12 @@ size_t hs_twophase_workspace_bytes(const hs_plan *p, int64_t batch)
     return ctrl_bytes(batch) + (size_t)s.R * (size_t)s.lay.slot_words * 4 + 256;
 }
 
-int hs_twophase_launches(const hs_plan *, int64_t) { return 2; }  // one memset node + one persistent kernel
+int hs_twophase_launches(const hs_plan *p, int64_t batch)
+{
+    const tp_sched s = make_sched(p, batch);
+    if (!s.plain) return 2;  // one memset node + one persistent kernel
+    return (int)((batch + s.R - 1) / s.R) * (s.nchunks > 0 ? 2 : 1);
+}
 
 bool hs_twophase_supported(const hs_plan *p, int64_t batch)
 {
