@@ -1,0 +1,485 @@
+// hs_interleaved.cu — eqs. 3 and 4 (CONVENTIONS.md C3, C4, C5) as a gather from a
+// spectrum-interleaved copy of a small group of spectra that lives in L2, run by ONE persistent kernel.
+//
+// Both variants read x(i n [+ j]) for i = 1..Hmax: a stride-i gather.  From the [batch][nbins] layout a warp of 32
+// consecutive n touches one 32-byte sector (and one 128-byte L1 line) per useful word for i >= 8, which is what bounds
+// the plain gather kernel (hs_greedy_gather.cu: one L1 wavefront per bin, 75-81 B/bin between L2 and the SMs).  Loop
+// inversion over the batch fixes it: G = 16 spectra are first copied into xT[k][g] (bin-major, the 16 spectra of a
+// group side by side: one 64-byte row per bin), and the gather runs with the lanes of a half-warp across the spectra
+// g, so every load instruction reads whole rows: full sectors whatever the stride, 4.06 (eq. 3) or 7.12 (eq. 4) words
+// per bin between L2 and the SMs.  A group's copy is 16 N floats (16 MiB at 2^18 bins) in a ring of R slots that stays
+// in L2: HBM sees x once (streamed, evict-first) and the outputs once (streaming stores).
+//
+// Work items, handed out in order from one global counter, step s = 0, 1, ..:
+//     T(s):   copy 512 bins x 16 spectra of group s into its ring slot; bins n >= N/2 have no harmonic but the first
+//             in range (S_H(n) = x(n) for every H), so their outputs are emitted right here, in the natural layout;
+//     G(s-2): 128 (bins below N/8) or 512 bins x 16 spectra of the gather for group s-2 (bins below N/2 only), low
+//             (= long) bins first;
+// T and G items of a step are interleaved in proportion, so that the HBM-bound copy and the L2/L1-bound gather overlap
+// on every SM.  A G item waits (acquire load on a per-group counter) until all T items of its group are done: those
+// were handed out a whole step earlier.  A T item waits until the gather of the group that used its ring slot last
+// (g - R, R = 4) is done: handed out at least a step earlier too.  Items only ever wait for items handed out EARLIER, and an
+// item is handed out to a CTA that is running, so the schedule cannot deadlock and needs no co-residency.
+//
+// Gather thread = (spectrum g of the group, C = 8 consecutive bins): 8 independent chains per thread hide Greedy's
+// serial dependence j -> address -> load, and the outputs of a thread are two float4 and two 4-byte stores.  Range
+// handling is warp-uniform (a warp owns 16 consecutive bins): harmonic i is in range for every lane iff
+// i (n_hi + 1) <= N.
+#include "hs_internal.cuh"
+#include "hs_ptx.cuh"
+
+namespace {
+
+constexpr int G = 16;                                   // spectra per group = floats per row of xT
+constexpr int C = 4;                                    // consecutive bins per gather thread (times 4 spectra)
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kWarpBins = 8 * C;                        // 32 bins per warp
+constexpr int kGTile = kWarps * kWarpBins;              // 256 bins per gather tile
+constexpr int kGSub = 2;                                // tiles per G item above the heavy region (bins >= N/8), 1 below
+constexpr int kLag = 2;                                 // the gather runs kLag steps behind the copy
+constexpr int kTBins = 512;                             // bins per T item
+constexpr int kTStride = kTBins + 4;                    // shared-memory row stride (floats) of the copy tile
+constexpr int kMaxRing = 4;
+
+struct il_params {
+    const float *x;
+    float *xT;          // ring of R slots, slot_words each
+    float *sums;
+    float *vmax;
+    uint8_t *amax;
+    int *ctrl;          // [0] work counter, [1] error flag, [2..5] wait statistics, [16 + g] T items done, [16 + groups + g] G items done
+    int64_t slot_words;
+    int N, B, groups, R;
+    int nT, nG;         // items per group
+    int nHeavy;         // the first nHeavy G items are single tiles (bins below ~N/8: 8 to 32 harmonics per bin)
+    int n_split;        // G items cover bins [0, n_split); T items emit the outputs of [n_split, N)
+};
+
+__device__ __forceinline__ float4 ld_stream(const float4 *p)   // read-once input: evict-first in L1 and L2
+{
+    float4 v;
+    asm volatile("ld.global.cs.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ int ld_acquire(const int *p)
+{
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// thread 0 only: wait until *cnt >= target (bounded: a bug must not hang the GPU; the error flag makes it visible)
+__device__ __forceinline__ void wait_count(const int *cnt, int target, int *err, int *stat)
+{
+    unsigned spins = 0;
+    while (ld_acquire(cnt) < target) {
+        __nanosleep(64);
+        if (++spins > (1u << 23)) {
+            atomicExch(err, 1);
+            break;
+        }
+    }
+    if (spins) {
+        atomicAdd(stat, 1);
+        atomicAdd(stat + 1, (int)(spins > 0x7fffu ? 0x7fffu : spins));
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ T item
+// xT[k][g] = x[b0 + g][k] for g < nb, 0 for nb <= g < G, k in [k0, k0 + 512) below N; outputs of the bins >= n_split.
+template <int L, int OUT>
+__device__ __forceinline__ void copy_item(const il_params &p, float *tile, int grp, int k0, float *__restrict__ xT)
+{
+    const int N = p.N;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t b0 = (int64_t)grp * G;
+    const int nb = (int)min((int64_t)G, (int64_t)p.B - b0);
+    constexpr int SPW = G / kWarps;                      // spectra per warp (2)
+    constexpr int Q = kTBins / 128;                      // float4 per lane per spectrum (4)
+    float4 v[SPW][Q];
+#pragma unroll
+    for (int s = 0; s < SPW; s++) {
+        const int g = warp * SPW + s;
+#pragma unroll
+        for (int q = 0; q < Q; q++) {
+            const int k = k0 + 4 * (lane + 32 * q);
+            v[s][q] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (g < nb && k < N) v[s][q] = ld_stream(reinterpret_cast<const float4 *>(p.x + (b0 + g) * N + k));
+        }
+    }
+#pragma unroll
+    for (int s = 0; s < SPW; s++) {
+        const int g = warp * SPW + s;
+#pragma unroll
+        for (int q = 0; q < Q; q++) {
+            const int kk = 4 * (lane + 32 * q);
+            // bit 3 of the column is flipped for the upper 8 spectra: makes the transposed reads below conflict-free
+            *reinterpret_cast<float4 *>(tile + g * kTStride + (kk ^ (g & 8))) = v[s][q];
+            const int k = k0 + kk;
+            if (k >= p.n_split && k < N && g < nb) {     // S_H(n) = x(n) for every H: emit in the natural layout
+                const int64_t row = (b0 + g) * N;
+                hs_emit<OUT> e0, e1, e2, e3;
+#pragma unroll
+                for (int l = 0; l < L; l++) {
+                    // h_l = x c_l is monotone in l: in reduced-only mode the first and the last level decide
+                    if (OUT == HS_OUT_REDUCED && l != 0 && l != L - 1) continue;
+                    const float4 h = make_float4(v[s][q].x * hs_norm(l), v[s][q].y * hs_norm(l), v[s][q].z * hs_norm(l),
+                                                 v[s][q].w * hs_norm(l));
+                    if (OUT & HS_OUT_FULL) hsptx::st_cs(reinterpret_cast<float4 *>(p.sums + (row * L + (int64_t)l * N + k)), h);
+                    if (OUT & HS_OUT_REDUCED) {
+                        e0.reduce(l, h.x);
+                        e1.reduce(l, h.y);
+                        e2.reduce(l, h.z);
+                        e3.reduce(l, h.w);
+                    }
+                }
+                if (OUT & HS_OUT_REDUCED) {
+                    hsptx::st_cs(reinterpret_cast<float4 *>(p.vmax + row + k), make_float4(e0.m, e1.m, e2.m, e3.m));
+                    hsptx::st_cs(reinterpret_cast<uint32_t *>(p.amax + row + k),
+                                 (uint32_t)e0.a | ((uint32_t)e1.a << 8) | ((uint32_t)e2.a << 16) | ((uint32_t)e3.a << 24));
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // thread t writes the float4 of spectra 4 (t % 4) .. +3 at bins k0 + t / 4 + 64 q
+    const int g4 = (threadIdx.x & 3) * 4;
+    const int sw = g4 & 8;
+#pragma unroll
+    for (int q = 0; q < kTBins / (kThreads / 4); q++) {
+        const int kk = q * (kThreads / 4) + (threadIdx.x >> 2);
+        if (k0 + kk < N) {
+            const float *t = tile + g4 * kTStride + (kk ^ sw);
+            const float4 o = make_float4(t[0], t[kTStride], t[2 * kTStride], t[3 * kTStride]);
+            *reinterpret_cast<float4 *>(xT + (int64_t)(k0 + kk) * G + g4) = o;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ G item
+// One tile of 256 bins x 16 spectra.  Thread = (4 spectra, 4 consecutive bins): one 16-byte load per bin and harmonic
+// serves four spectra; a warp owns 32 consecutive bins, and per output row it stores 128 contiguous bytes of maxima
+// and 32 of best levels.
+template <int L, int OUT>
+__device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_cta, const float *__restrict__ xT)
+{
+    const int N = p.N;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int q4 = lane & 3;                                           // spectra 4 q4 .. 4 q4 + 3 of the group
+    const int n_w = n_cta + warp * kWarpBins;                          // first bin of this warp
+    const int n_end = min(N, p.n_split);                               // bins [n_end, N) belong to the T items
+    if (n_w >= n_end) return;                                          // (warp-uniform)
+    const int n0 = n_w + (lane >> 2) * C;                              // first bin of this thread
+    const int n_hi1 = min(n_w + kWarpBins, n_end);                     // one past the warp's last bin
+    const bool whole = n_w + kWarpBins <= n_end;                       // every lane's C bins exist
+    const int64_t b0 = (int64_t)grp * G + 4 * q4;                      // first of this thread's spectra
+    const float4 *__restrict__ xq = reinterpret_cast<const float4 *>(xT) + q4;   // row k: xq[k * (G / 4)]
+    constexpr int RS = G / 4;                                          // float4 per row
+
+    float4 S[C];
+    hs_emit<OUT> e[C][4];
+
+    auto emit = [&](int l) {
+        const float c = hs_norm(l);
+#pragma unroll
+        for (int k = 0; k < C; k++) {
+            if (OUT & HS_OUT_REDUCED) {
+                e[k][0].reduce(l, S[k].x * c);
+                e[k][1].reduce(l, S[k].y * c);
+                e[k][2].reduce(l, S[k].z * c);
+                e[k][3].reduce(l, S[k].w * c);
+            }
+        }
+        if (OUT & HS_OUT_FULL) {
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                if (b0 + q < p.B) {
+                    float *pl = p.sums + ((b0 + q) * L + l) * N + n0;
+                    const float h0 = (q == 0 ? S[0].x : q == 1 ? S[0].y : q == 2 ? S[0].z : S[0].w) * c;
+                    const float h1 = (q == 0 ? S[1].x : q == 1 ? S[1].y : q == 2 ? S[1].z : S[1].w) * c;
+                    const float h2 = (q == 0 ? S[2].x : q == 1 ? S[2].y : q == 2 ? S[2].z : S[2].w) * c;
+                    const float h3 = (q == 0 ? S[3].x : q == 1 ? S[3].y : q == 2 ? S[3].z : S[3].w) * c;
+                    if (whole) {
+                        hsptx::st_cs(reinterpret_cast<float4 *>(pl), make_float4(h0, h1, h2, h3));
+                    } else {
+                        if (n0 + 0 < n_end) hsptx::st_cs(pl + 0, h0);
+                        if (n0 + 1 < n_end) hsptx::st_cs(pl + 1, h1);
+                        if (n0 + 2 < n_end) hsptx::st_cs(pl + 2, h2);
+                        if (n0 + 3 < n_end) hsptx::st_cs(pl + 3, h3);
+                    }
+                }
+            }
+        }
+    };
+    auto add = [](float4 &a, const float4 &b) {
+        a.x += b.x;
+        a.y += b.y;
+        a.z += b.z;
+        a.w += b.w;
+    };
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+
+    // harmonic 1
+#pragma unroll
+    for (int k = 0; k < C; k++) S[k] = (whole || n0 + k < N) ? hsptx::ld_cg(xq + (n0 + k) * RS) : zero;
+    emit(0);
+
+    // harmonics i and i + 1, both in range for every lane: no bounds checks, 8 independent 16-byte loads in flight
+    auto step_safe2 = [&](int i) {
+        const int base = i * n0, base2 = base + n0;
+        float4 a[C], b[C];
+#pragma unroll
+        for (int k = 0; k < C; k++) {
+            a[k] = hsptx::ld_cg(xq + (base + k * i) * RS);
+            b[k] = hsptx::ld_cg(xq + (base2 + k * (i + 1)) * RS);
+        }
+#pragma unroll
+        for (int k = 0; k < C; k++) {
+            add(S[k], a[k]);
+            add(S[k], b[k]);
+        }
+    };
+    auto step_safe = [&](int i) {
+        const int base = i * n0;
+        float4 a[C];
+#pragma unroll
+        for (int k = 0; k < C; k++) a[k] = hsptx::ld_cg(xq + (base + k * i) * RS);
+#pragma unroll
+        for (int k = 0; k < C; k++) add(S[k], a[k]);
+    };
+    // harmonic i straddling the end of the spectrum: zero padding (C5)
+    auto step_edge = [&](int i) {
+        const int base = i * n0;
+#pragma unroll
+        for (int k = 0; k < C; k++) {
+            const int r = base + k * i;
+            add(S[k], r < N ? hsptx::ld_cg(xq + r * RS) : zero);
+        }
+    };
+
+    bool tail = false;   // levels skipped because none of their harmonics is in range for the warp (reduced only)
+#pragma unroll
+    for (int l = 1; l < L; l++) {
+        const int lo = (1 << (l - 1)) + 1, hi = 1 << l;
+        if (lo * n_w < N) {
+            int i = lo;
+            if (whole) {
+                for (; i + 1 <= hi && (i + 1) * n_hi1 <= N; i += 2) step_safe2(i);
+                for (; i <= hi && i * n_hi1 <= N; i++) step_safe(i);
+            }
+            for (; i <= hi && i * n_w < N; i++) step_edge(i);
+            emit(l);
+        } else if (OUT != HS_OUT_REDUCED) {
+            emit(l);
+        } else {
+            tail = true;
+        }
+    }
+    // With S unchanged over the skipped levels h_l = S c_l is monotone in l: testing the last level alone is enough.
+    if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
+
+    if (OUT & HS_OUT_REDUCED) {
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            if (b0 + q < p.B) {
+                float *pm = p.vmax + (b0 + q) * N + n0;
+                uint8_t *pa = p.amax + (b0 + q) * N + n0;
+                if (whole) {
+                    hsptx::st_cs(reinterpret_cast<float4 *>(pm), make_float4(e[0][q].m, e[1][q].m, e[2][q].m, e[3][q].m));
+                    hsptx::st_cs(reinterpret_cast<uint32_t *>(pa), (uint32_t)e[0][q].a | ((uint32_t)e[1][q].a << 8) |
+                                                                       ((uint32_t)e[2][q].a << 16) | ((uint32_t)e[3][q].a << 24));
+                } else {
+#pragma unroll
+                    for (int k = 0; k < C; k++) {
+                        if (n0 + k < n_end) {
+                            hsptx::st_cs(pm + k, e[k][q].m);
+                            hsptx::st_cs(pa + k, (uint8_t)e[k][q].a);
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ persistent kernel
+template <int L, int OUT>
+__global__ void __launch_bounds__(kThreads, 2)
+il_persistent_kernel(const __grid_constant__ il_params p)
+{
+    __shared__ __align__(16) float tile[G * kTStride];
+    __shared__ int s_item;
+    int *queue = p.ctrl, *err = p.ctrl + 1;
+    int *doneT = p.ctrl + 16, *doneG = p.ctrl + 16 + p.groups;
+    const int per = p.nT + p.nG;
+    const int total = (p.groups + kLag) * per;
+    int lastT = -1, lastG = -1;                                         // thread 0: groups already seen complete
+    if (threadIdx.x == 0) s_item = atomicAdd(queue, 1);
+    __syncthreads();
+    int item = s_item;
+    while (item < total) {
+        int next = 0;
+        if (threadIdx.x == 0) next = atomicAdd(queue, 1);               // in flight while this item runs
+        const int s = item / per, r = item - s * per;
+        // T and G items of a step interleaved in proportion nT : nG
+        const int t_before = (int)(((int64_t)r * p.nT) / per), t_after = (int)(((int64_t)(r + 1) * p.nT) / per);
+        if (t_after > t_before) {                                       // ---- T item t_before of group s
+            if (s < p.groups) {
+                float *xT = p.xT + (int64_t)(s % p.R) * p.slot_words;
+                if (threadIdx.x == 0 && s >= p.R && p.nG > 0 && lastG < s - p.R) {
+                    wait_count(doneG + (s - p.R), p.nG, err, p.ctrl + 2);
+                    lastG = s - p.R;
+                }
+                __syncthreads();
+                copy_item<L, OUT>(p, tile, s, t_before * kTBins, xT);
+                __syncthreads();                                        // all stores of the CTA are ordered before ...
+                if (threadIdx.x == 0) {
+                    __threadfence();                                    // ... thread 0's release at gpu scope
+                    atomicAdd(doneT + s, 1);
+                }
+            }
+        } else if (s >= kLag) {                                         // ---- G item (r - t_before) of group s - kLag
+            const int grp = s - kLag;
+            const float *xT = p.xT + (int64_t)(grp % p.R) * p.slot_words;
+            if (threadIdx.x == 0 && lastT < grp) {
+                wait_count(doneT + grp, p.nT, err, p.ctrl + 4);
+                lastT = grp;
+            }
+            __syncthreads();
+            const int q = r - t_before;
+            if (q < p.nHeavy) {
+                gather_item<L, OUT>(p, grp, q * kGTile, xT);
+            } else {
+#pragma unroll 1
+                for (int sub = 0; sub < kGSub; sub++)
+                    gather_item<L, OUT>(p, grp, (p.nHeavy + (q - p.nHeavy) * kGSub + sub) * kGTile, xT);
+            }
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                __threadfence();
+                atomicAdd(doneG + grp, 1);
+            }
+        }
+        if (threadIdx.x == 0) s_item = next;
+        __syncthreads();                                                // s_item and the tile are reused
+        item = s_item;
+        __syncthreads();
+    }
+}
+
+struct il_sched {
+    int groups, R, nT, nG, nHeavy, n_split;
+    int64_t slot_words;
+};
+
+il_sched make_sched(const hs_plan *p, int64_t batch)
+{
+    il_sched s{};
+    const int N = (int)p->nbins;
+    s.groups = (int)((batch + G - 1) / G);
+    s.R = s.groups < kMaxRing ? s.groups : kMaxRing;
+    s.nT = (N + kTBins - 1) / kTBins;
+    // bins n >= N/2 have S_H(n) = x(n): the T items emit them.  The split is a multiple of the T tile.
+    const int half = (N + 1) / 2;
+    int split = (half + kTBins - 1) / kTBins * kTBins;
+    if (p->Hmax == 1) split = 0;                                       // nothing to gather at all
+    if (split > N) split = (N + kGTile - 1) / kGTile * kGTile;          // (only spectra shorter than a T tile)
+    s.n_split = split;
+    const int tiles = (((split < N) ? split : N) + kGTile - 1) / kGTile;
+    s.nHeavy = (N / 8 + kGTile - 1) / kGTile;
+    if (s.nHeavy > tiles) s.nHeavy = tiles;
+    s.nG = s.nHeavy + (tiles - s.nHeavy + kGSub - 1) / kGSub;
+    s.slot_words = ((int64_t)N * G + 63) & ~(int64_t)63;
+    return s;
+}
+
+size_t ctrl_bytes(int groups) { return ((size_t)(16 + 2 * (size_t)groups) * sizeof(int) + 255) / 256 * 256; }
+
+template <int L, int OUT>
+int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    const il_sched s = make_sched(p, batch);
+    il_params prm{};
+    prm.x = buf.x;
+    prm.ctrl = static_cast<int *>(ws);
+    prm.xT = reinterpret_cast<float *>(static_cast<char *>(ws) + ctrl_bytes(s.groups));
+    prm.sums = buf.sums;
+    prm.vmax = buf.vmax;
+    prm.amax = buf.amax;
+    prm.slot_words = s.slot_words;
+    prm.N = (int)p->nbins;
+    prm.B = (int)batch;
+    prm.groups = s.groups;
+    prm.R = s.R;
+    prm.nT = s.nT;
+    prm.nG = s.nG;
+    prm.nHeavy = s.nHeavy;
+    prm.n_split = s.n_split;
+    auto kern = il_persistent_kernel<L, OUT>;
+    static int ctas_per_sm = 0;
+    if (ctas_per_sm == 0) {
+        int occ = 0;
+        HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, 0));
+        ctas_per_sm = occ > 0 ? occ : 1;
+    }
+    HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(s.groups), stream));
+    const int64_t total = (int64_t)(s.groups + kLag) * (s.nT + s.nG);
+    const int64_t slots = (int64_t)p->sm_count * ctas_per_sm;
+    kern<<<(unsigned)(total < slots ? total : slots), kThreads, 0, stream>>>(prm);
+    HS_CUDA_OK(cudaGetLastError());
+    return HS_OK;
+}
+
+template <int L>
+int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    switch (p->out_mode) {
+        case HS_OUT_FULL: return launch<L, HS_OUT_FULL>(p, buf, batch, ws, stream);
+        case HS_OUT_REDUCED: return launch<L, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
+        default: return launch<L, HS_OUT_BOTH>(p, buf, batch, ws, stream);
+    }
+}
+
+int by_level(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    switch (p->L) {
+        case 1: return by_out<1>(p, buf, batch, ws, stream);
+        case 2: return by_out<2>(p, buf, batch, ws, stream);
+        case 3: return by_out<3>(p, buf, batch, ws, stream);
+        case 4: return by_out<4>(p, buf, batch, ws, stream);
+        case 5: return by_out<5>(p, buf, batch, ws, stream);
+        default: return by_out<6>(p, buf, batch, ws, stream);
+    }
+}
+
+}  // namespace
+
+// The interleaved copies of a ring of groups have to stay in L2 (126 MB): at most 16 MiB per slot, i.e. spectra of up
+// to 2^18 bins; longer spectra take the plain gather kernel.  Item numbers are 32-bit.
+bool hs_interleaved_supported(const hs_plan *p)
+{
+    if (p->variant != HS_FREQBIN) return false;
+    if (p->nbins > ((int64_t)1 << 18)) return false;
+    const il_sched s = make_sched(p, p->batch);
+    return ((int64_t)s.groups + kLag) * (s.nT + s.nG) < ((int64_t)1 << 30);
+}
+
+size_t hs_interleaved_workspace_bytes(const hs_plan *p, int64_t batch)
+{
+    const il_sched s = make_sched(p, batch);
+    return ctrl_bytes(s.groups) + (size_t)s.R * (size_t)s.slot_words * sizeof(float) + 256;
+}
+
+int hs_interleaved_launches(const hs_plan *p, int64_t batch)
+{
+    (void)p;
+    (void)batch;
+    return 2;   // one memset node + one persistent kernel
+}
+
+int hs_interleaved_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    if (!ws) HS_FAIL(HS_ERR_WORKSPACE);
+    return by_level(p, buf, batch, ws, stream);
+}

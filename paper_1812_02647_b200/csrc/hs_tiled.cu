@@ -3,23 +3,35 @@
 #include "hs_internal.cuh"
 
 namespace {
-// Max always runs two-phase; freq-bin runs two-phase only when asked to (HS_ALGO_TWOPHASE), else the gather kernel.
+// Max always runs two-phase; freq-bin runs two-phase only when asked to (HS_ALGO_TWOPHASE).
 bool two_phase(const hs_plan *p)
 {
     return p->variant == HS_MAX || (p->variant == HS_FREQBIN && p->algo_req == HS_ALGO_TWOPHASE);
 }
+// freq-bin and Greedy gather from the spectrum-interleaved group copies when they fit L2, unless the plain gather is asked for
+bool interleaved(const hs_plan *p)
+{
+    return !two_phase(p) && p->algo_req != HS_ALGO_GATHER && hs_interleaved_supported(p);
+}
 }  // namespace
-bool hs_tiled_supported(const hs_plan *p) { return !two_phase(p) || hs_twophase_supported(p, p->batch); }
+bool hs_tiled_supported(const hs_plan *p)
+{
+    if (p->algo_req == HS_ALGO_GATHER && p->variant != HS_FREQBIN && p->variant != HS_GREEDY) return false;
+    return !two_phase(p) || hs_twophase_supported(p, p->batch);
+}
 
 size_t hs_tiled_workspace_bytes(const hs_plan *p, int64_t batch)
 {
-    return two_phase(p) ? hs_twophase_workspace_bytes(p, batch) : 0;
+    if (two_phase(p)) return hs_twophase_workspace_bytes(p, batch);
+    if (interleaved(p)) return hs_interleaved_workspace_bytes(p, batch);
+    return 0;
 }
 
 int hs_tiled_launches(const hs_plan *p, int64_t batch)
 {
     if (p->variant == HS_STANDARD) return hs_standard_tiled_launches(p, batch);
     if (two_phase(p)) return hs_twophase_launches(p, batch);
+    if (interleaved(p)) return hs_interleaved_launches(p, batch);
     return hs_greedy_gather_launches(p, batch);
 }
 
@@ -27,5 +39,6 @@ int hs_launch_tiled(const hs_plan *p, const hs_buffers &buf, int64_t batch, void
 {
     if (p->variant == HS_STANDARD) return hs_standard_tiled_launch(p, buf, batch, stream);
     if (two_phase(p)) return hs_twophase_launch(p, buf, batch, ws, stream);
+    if (interleaved(p)) return hs_interleaved_launch(p, buf, batch, ws, stream);
     return hs_greedy_gather_launch(p, buf, batch, stream);
 }

@@ -15,7 +15,7 @@ from parity import argmax_from_levels, check_argmax, check_sums
 pytestmark = pytest.mark.gpu
 
 VARIANTS = ["standard", "max", "freqbin", "greedy"]
-ALGOS = ["direct", "tiled", "twophase"]
+ALGOS = ["direct", "tiled", "twophase", "gather"]
 
 
 @pytest.fixture(scope="module")
@@ -30,9 +30,11 @@ def hs():
 
 def make_plan(hs, N, B, Hmax, variant, out_mode, algo):
     plan = hs.hs_plan_create(N, B, Hmax, variant, out_mode)
-    if algo in ("tiled", "twophase"):
+    if algo in ("tiled", "twophase", "gather"):
         if algo == "twophase" and variant != "freqbin":
             pytest.skip("two-phase is a separate choice for freq-bin only (Max: same as tiled)")
+        if algo == "gather" and variant not in ("freqbin", "greedy"):
+            pytest.skip("the plain gather kernel covers eqs. 3-4 only")
         try:
             plan.set_algo(algo)
         except hs.HsError:
@@ -73,7 +75,7 @@ def run_and_compare(hs, oracle, x_np, Hmax, variant, out_mode, algo, check_j=Tru
 @pytest.mark.parametrize("variant", VARIANTS)
 def test_small_and_ragged_sizes(hs, oracle, variant, algo):
     rng = np.random.default_rng(1)
-    for N, B in ((4, 1), (8, 3), (12, 1), (36, 2), (100, 1), (1000, 3), (4100, 2), (33000, 1)):
+    for N, B in ((4, 1), (8, 3), (12, 1), (36, 2), (100, 1), (1000, 3), (4100, 2), (33000, 1), (2052, 37)):
         x = (rng.standard_exponential((B, N)) - 1).astype(np.float32)
         run_and_compare(hs, oracle, x, 32, variant, "both", algo)
 
