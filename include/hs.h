@@ -58,8 +58,11 @@ enum hs_algo {
                            eq. 2 two-phase through a workspace; eqs. 3-4 gather from a spectrum-interleaved copy of
                            16 spectra at a time that stays in L2 (workspace)                                        */
     HS_ALGO_TWOPHASE = 3, /* eqs. 2-3 only: the two-phase kernel (for eq. 2 the same as HS_ALGO_TILED)              */
-    HS_ALGO_GATHER = 4    /* eqs. 3-4 only: the range-skipping gather straight from x (no workspace); what
+    HS_ALGO_GATHER = 4,   /* eqs. 3-4 only: the range-skipping gather straight from x (no workspace); what
                              HS_ALGO_TILED itself uses for spectra too long for the interleaved group copy           */
+    HS_ALGO_GROUPED = 5   /* eqs. 2-3 only: two phases per spectrum by a static group of co-resident CTAs, the
+                             per-harmonic arrays of a spectrum live in one L2-resident workspace slot per group
+                             (cooperative launch); what HS_ALGO_TILED uses for eq. 2 when a slot fits L2            */
 };
 
 /*

@@ -15,7 +15,7 @@ from parity import argmax_from_levels, check_argmax, check_sums
 pytestmark = pytest.mark.gpu
 
 VARIANTS = ["standard", "max", "freqbin", "greedy"]
-ALGOS = ["direct", "tiled", "twophase", "gather"]
+ALGOS = ["direct", "tiled", "twophase", "gather", "grouped"]
 
 
 @pytest.fixture(scope="module")
@@ -30,9 +30,9 @@ def hs():
 
 def make_plan(hs, N, B, Hmax, variant, out_mode, algo):
     plan = hs.hs_plan_create(N, B, Hmax, variant, out_mode)
-    if algo in ("tiled", "twophase", "gather"):
-        if algo == "twophase" and variant != "freqbin":
-            pytest.skip("two-phase is a separate choice for freq-bin only (Max: same as tiled)")
+    if algo in ("tiled", "twophase", "gather", "grouped"):
+        if algo in ("twophase", "grouped") and variant not in ("max", "freqbin"):
+            pytest.skip("the two-phase kernels cover eqs. 2-3 only")
         if algo == "gather" and variant not in ("freqbin", "greedy"):
             pytest.skip("the plain gather kernel covers eqs. 3-4 only")
         try:
