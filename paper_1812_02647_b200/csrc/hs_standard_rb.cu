@@ -1,0 +1,290 @@
+// hs_standard_rb.cu — eq. 1 (CONVENTIONS.md C1) at Hmax = 32, reduced output, register blocked.
+//
+// The term of harmonic i = 1..32 at output n is x[(n i + 16) >> 5].  With n = 32 m + r the index is m i + c(r, i),
+// c(r, i) = (r i + 16) >> 5 in [0, i]: a THREAD that owns the 32 consecutive outputs 32 m .. 32 m + 31 reads, for
+// harmonic i, only the i + 1 words x[m i .. m i + i], and every one of its 1024 (r, i) terms has a compile-time register
+// index.  That is 17.5 shared-memory words per output instead of the 32 of a lane-per-output mapping (hs_standard_tiled.cu),
+// which is what bounds eq. 1: the path is limited by shared-memory bandwidth and L2 -> SM fill, not by HBM.
+//
+// A CTA of 128 threads takes tiles of 4096 consecutive outputs (lane = m) and streams the 32 harmonics through a ring
+// of shared-memory slots in dyadic level order 32 | 16 | 8 24 | 4 12 20 28 | 2 6 .. 30 | 1 3 .. 31, so that one running
+// sum per output serves all six levels (eq. 1 is cumulative over dyadic H).  The window of harmonic i for the tile is
+// the contiguous range x[n0 i / 32 .. (n0 + 4096) i / 32]: 128 i + 1 words.
+//   * i not a multiple of 8: one TMA bulk copy per window (cp.async.bulk, UBLKCP) onto the slot's mbarrier.  Lane stride
+//     is i words: conflict-free 4-byte loads for odd i, 8-byte loads for i = 2 (mod 4), 16-byte loads for i = 4 (mod 8).
+//   * i = 8, 16, 24, 32: a lane stride of i words would hit the same banks, so the window is copied by cp.async
+//     (16 bytes per thread) into rows of i + 4 words: one pad unit per thread row makes the 16-byte loads conflict-free.
+// The warp that finishes with a slot last refills it with the window three stages ahead (a counter per slot in shared
+// memory, one mbarrier per slot for the arrival of the data: no CTA-wide barrier anywhere); the ring runs across tiles.
+// The reduced outputs of a thread (32 consecutive floats) are transposed through shared memory per warp so that the
+// global stores are coalesced.
+#include <utility>
+
+#include "hs_internal.cuh"
+#include "hs_ptx.cuh"
+
+namespace {
+
+constexpr int kT = 4096;                  // outputs per tile
+constexpr int kNT = 128;                  // threads per CTA: one per 32 outputs
+constexpr int kSlot = 5128;               // words per ring slot: the largest stage (padded windows of i = 8 and 24)
+constexpr int kSlots = 3;
+constexpr int kOutRow = 20;               // words per lane row of the output transposition buffer (16 + 4 pad)
+constexpr int kCtasPerSm = 3;
+constexpr int kStages = 17;
+
+// A stage brings the windows of one or two harmonics (about 4100 words, so the stages are evenly sized), in dyadic
+// level order: 32 | 16 | 8 24 | 4 28, 12 20 | 2 30, 6 26, 10 22, 14 18 | 1 31, 3 29, .., 15 17
+__host__ __device__ constexpr int stream_a(int s)
+{
+    return s == 0 ? 32 : s == 1 ? 16 : s == 2 ? 8 : s == 3 ? 4 : s == 4 ? 12 : s < 9 ? 2 + 4 * (s - 5) : 1 + 2 * (s - 9);
+}
+__host__ __device__ constexpr int stream_b(int s) { return s < 2 ? 0 : 32 - stream_a(s); }
+// level completed by stage s, or -1
+__host__ __device__ constexpr int level_after(int s)
+{
+    return s == 0 ? 0 : s == 1 ? 1 : s == 2 ? 2 : s == 4 ? 3 : s == 8 ? 4 : s == 16 ? 5 : -1;
+}
+__host__ __device__ constexpr bool is_padded(int i) { return (i & 7) == 0; }
+__host__ __device__ constexpr int cidx(int r, int i) { return (r * i + 16) >> 5; }
+// words the window of harmonic i occupies in a slot (padded rows of i + 4 words, or 128 i + 1 words rounded up to 16 bytes)
+__host__ __device__ constexpr int slot_words(int i) { return is_padded(i) ? 128 * (i + 4) + (i <= 16 ? 4 : 0) : 128 * i + 4; }
+
+struct rb_params {
+    const float *x;
+    float *vmax;
+    uint8_t *amax;
+    int N;
+    int tiles_per_spectrum;
+    int64_t tiles;   // total
+};
+
+__device__ __forceinline__ void cp_async16(void *dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(hsptx::smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
+
+// S[r] (+)= x[m i + c(r, i)] for the thread's 32 outputs, window of harmonic I staged in `slot` (lane = tile-local m)
+template <int I>
+__device__ __forceinline__ void accumulate(const float *__restrict__ slot, int mloc, float (&S)[32])
+{
+    float w[I + 4];
+    if constexpr (is_padded(I)) {
+        const float *__restrict__ row = slot + mloc * (I + 4);
+#pragma unroll
+        for (int q = 0; q < I / 4; q++) {
+            const float4 u = *reinterpret_cast<const float4 *>(row + 4 * q);
+            w[4 * q] = u.x, w[4 * q + 1] = u.y, w[4 * q + 2] = u.z, w[4 * q + 3] = u.w;
+        }
+        if constexpr (I <= 16) w[I] = row[I + 4];               // first word of the next thread's row
+    } else if constexpr (I % 4 == 0) {
+        const float *__restrict__ row = slot + mloc * I;
+#pragma unroll
+        for (int q = 0; q <= I / 4; q++) {
+            const float4 u = *reinterpret_cast<const float4 *>(row + 4 * q);
+            w[4 * q] = u.x, w[4 * q + 1] = u.y, w[4 * q + 2] = u.z, w[4 * q + 3] = u.w;
+        }
+    } else if constexpr (I % 2 == 0) {
+        const float *__restrict__ row = slot + mloc * I;
+#pragma unroll
+        for (int q = 0; q <= I / 2; q++) {
+            const float2 u = *reinterpret_cast<const float2 *>(row + 2 * q);
+            w[2 * q] = u.x, w[2 * q + 1] = u.y;
+        }
+    } else {
+        const float *__restrict__ row = slot + mloc * I;
+#pragma unroll
+        for (int k = 0; k <= I; k++) w[k] = row[k];
+    }
+#pragma unroll
+    for (int r = 0; r < 32; r++) {
+        if constexpr (I == 32) S[r] = w[cidx(r, I)];             // first harmonic of a tile: starts the running sums
+        else S[r] += w[cidx(r, I)];
+    }
+}
+
+// level l complete: h = S c_l, running maximum and best level (C8: a later level wins only if strictly greater)
+template <int LV>
+__device__ __forceinline__ void emit_level(const float (&S)[32], float (&m)[32], int (&a)[32])
+{
+#pragma unroll
+    for (int r = 0; r < 32; r++) {
+        const float h = S[r] * hs_norm(LV);
+        if (LV == 0) {
+            m[r] = h;
+            a[r] = 0;
+        } else if (h > m[r]) {
+            m[r] = h;
+            a[r] = LV;
+        }
+    }
+}
+
+template <class F, int... s>
+__device__ __forceinline__ void for_each_stage(F &f, std::integer_sequence<int, s...>)
+{
+    (f(std::integral_constant<int, s>{}), ...);
+}
+
+__global__ void __launch_bounds__(kNT, kCtasPerSm)
+rb_kernel(const __grid_constant__ rb_params p)
+{
+    extern __shared__ __align__(128) float smem[];
+    __shared__ __align__(8) uint64_t full[kSlots];
+    float *ring = smem;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float *ob = smem + kSlots * kSlot + warp * (32 * kOutRow);
+    const int N = p.N;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < kSlots; s++) hsptx::mbar_init(&full[s], 1);
+        hsptx::mbar_fence_init();
+    }
+    __syncthreads();
+
+    // tiles blockIdx.x, blockIdx.x + gridDim.x, ..: (spectrum, tile in spectrum) advanced without divisions
+    const int tps = p.tiles_per_spectrum;
+    const int step_b = (int)(gridDim.x / (unsigned)tps), step_t = (int)(gridDim.x % (unsigned)tps);
+    int cb = (int)(blockIdx.x / (unsigned)tps), ct = (int)(blockIdx.x % (unsigned)tps);
+    const int ktiles = (int)(blockIdx.x < p.tiles ? (p.tiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0);
+    auto next_tile = [&](int &bb, int &tt) {
+        bb += step_b;
+        tt += step_t;
+        if (tt >= tps) {
+            tt -= tps;
+            bb++;
+        }
+    };
+
+    // start the copies of stage SC of tile (spectrum ib, tile it) into slot `islot` (the stage is a compile-time
+    // constant: the stage that issues it is known); every thread commits one cp.async group per stage
+    auto issue = [&](auto sc, int ib, int it, int islot, bool live) {
+        constexpr int SC = decltype(sc)::value, IA = stream_a(SC), IB = stream_b(SC);
+        if (live) {
+            float *dst = ring + islot * kSlot;
+            const float *xb = p.x + ((int64_t)ib * N + (int64_t)it * (kT / 32 * IA));        // x[n0 IA / 32]: 16-byte aligned
+            if constexpr (is_padded(IA)) {
+                auto copy_padded = [&](auto ic, float *d, const float *src) {
+                    constexpr int I = decltype(ic)::value, units = 32 * I + (I <= 16 ? 1 : 0), rowu = I / 4;
+#pragma unroll
+                    for (int u0 = 0; u0 < units; u0 += kNT) {
+                        const int u = u0 + threadIdx.x;
+                        if (u0 + kNT <= units || u < units) cp_async16(d + 4 * (u + u / rowu), src + 4 * u);
+                    }
+                };
+                copy_padded(std::integral_constant<int, IA>{}, dst, xb);
+                if constexpr (IB != 0)
+                    copy_padded(std::integral_constant<int, IB == 0 ? 8 : IB>{}, dst + slot_words(IA),
+                                xb + (int64_t)it * (kT / 32 * (IB - IA)));
+            } else if (threadIdx.x == 0) {
+                constexpr uint32_t bytesA = (uint32_t)slot_words(IA) * 4u, bytesB = (uint32_t)slot_words(IB) * 4u;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the slot was last read by ordinary loads
+                hsptx::mbar_arrive_expect_tx(&full[islot], bytesA + bytesB);
+                hsptx::bulk_g2s(dst, xb, bytesA, &full[islot]);
+                hsptx::bulk_g2s(dst + slot_words(IA), xb + (int64_t)it * (kT / 32 * (IB - IA)), bytesB, &full[islot]);
+            }
+        }
+        cp_async_commit();
+    };
+
+    issue(std::integral_constant<int, 0>{}, cb, ct, 0, ktiles > 0);
+    issue(std::integral_constant<int, 1>{}, cb, ct, 1, ktiles > 0);
+    issue(std::integral_constant<int, 2>{}, cb, ct, 2, ktiles > 0);
+
+    uint32_t phase = 0u;                                                  // bit s: parity of the next wait on full[s]
+    float S[32], m[32];
+    int a[32];
+    int slot = 0;
+    for (int k = 0; k < ktiles; k++) {
+        const int64_t b = cb;
+        const int n0 = ct * kT;
+        int nb = cb, nt = ct;                                             // the CTA's next tile
+        next_tile(nb, nt);
+        const bool more = k + 1 < ktiles;
+        auto stage = [&](auto sc) {
+            constexpr int s = decltype(sc)::value, IA = stream_a(s), IB = stream_b(s), LV = level_after(s);
+            if constexpr (is_padded(IA)) {
+                cp_async_wait<kSlots - 1>();
+                __syncthreads();
+            } else {
+                hsptx::mbar_wait(&full[slot], (phase >> slot) & 1u);
+                phase ^= 1u << slot;
+            }
+            accumulate<IA>(ring + slot * kSlot, threadIdx.x, S);
+            if constexpr (IB != 0) accumulate<IB == 0 ? 1 : IB>(ring + slot * kSlot + slot_words(IA), threadIdx.x, S);
+            if constexpr (LV >= 0) emit_level<LV>(S, m, a);
+            __syncthreads();                                              // the slot is free: refill it with stage s + 3
+            constexpr int s3 = (s + kSlots) % kStages;
+            if constexpr (s + kSlots < kStages) issue(std::integral_constant<int, s3>{}, cb, ct, slot, true);
+            else issue(std::integral_constant<int, s3>{}, nb, nt, slot, more);
+            slot = slot == kSlots - 1 ? 0 : slot + 1;
+        };
+        for_each_stage(stage, std::make_integer_sequence<int, kStages>{});
+        cb = nb;
+        ct = nt;
+
+        // ---- outputs of the tile: thread holds bins nw0 + 32 lane + [0, 32)
+        const int64_t base = b * N + n0 + warp * 1024;
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+#pragma unroll
+            for (int q = 0; q < 4; q++)
+                *reinterpret_cast<float4 *>(ob + lane * kOutRow + 4 * q) =
+                    make_float4(m[16 * h + 4 * q], m[16 * h + 4 * q + 1], m[16 * h + 4 * q + 2], m[16 * h + 4 * q + 3]);
+            __syncwarp();
+#pragma unroll
+            for (int kk = 0; kk < 4; kk++) {
+                const int row = 8 * kk + (lane & 7), q = lane >> 3;
+                const float4 v = *reinterpret_cast<const float4 *>(ob + row * kOutRow + 4 * q);
+                hsptx::st_cs(reinterpret_cast<float4 *>(p.vmax + base + 32 * row + 16 * h + 4 * q), v);
+            }
+            __syncwarp();
+            uint32_t pk[4];
+#pragma unroll
+            for (int q = 0; q < 4; q++)
+                pk[q] = (uint32_t)a[16 * h + 4 * q] | ((uint32_t)a[16 * h + 4 * q + 1] << 8) |
+                        ((uint32_t)a[16 * h + 4 * q + 2] << 16) | ((uint32_t)a[16 * h + 4 * q + 3] << 24);
+            asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p.amax + base + 32 * lane + 16 * h), "r"(pk[0]),
+                         "r"(pk[1]), "r"(pk[2]), "r"(pk[3])
+                         : "memory");
+        }
+    }
+    asm volatile("cp.async.wait_all;" ::: "memory");
+}
+
+}  // namespace
+
+// Hmax = 32, reduced output only, spectra made of whole 4096-bin tiles; everything else takes hs_standard_tiled.cu.
+bool hs_standard_rb_supported(const hs_plan *p)
+{
+    return p->variant == HS_STANDARD && p->Hmax == 32 && p->out_mode == HS_OUT_REDUCED && p->nbins % kT == 0;
+}
+
+int hs_standard_rb_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+{
+    rb_params prm{};
+    prm.x = buf.x;
+    prm.vmax = buf.vmax;
+    prm.amax = buf.amax;
+    prm.N = (int)p->nbins;
+    prm.tiles_per_spectrum = (int)(p->nbins / kT);
+    prm.tiles = batch * prm.tiles_per_spectrum;
+    const size_t smem = (size_t)(kSlots * kSlot + (kNT / 32) * 32 * kOutRow) * sizeof(float);
+    static bool configured = false;
+    if (!configured) {
+        HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = true;
+    }
+    const int64_t slots = (int64_t)p->sm_count * kCtasPerSm;
+    const unsigned grid = (unsigned)(prm.tiles < slots ? prm.tiles : slots);
+    rb_kernel<<<grid, kNT, smem, stream>>>(prm);
+    HS_CUDA_OK(cudaGetLastError());
+    return HS_OK;
+}

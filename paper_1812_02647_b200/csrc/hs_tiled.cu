@@ -40,7 +40,7 @@ size_t hs_tiled_workspace_bytes(const hs_plan *p, int64_t batch)
 
 int hs_tiled_launches(const hs_plan *p, int64_t batch)
 {
-    if (p->variant == HS_STANDARD) return hs_standard_tiled_launches(p, batch);
+    if (p->variant == HS_STANDARD) return hs_standard_rb_supported(p) ? 1 : hs_standard_tiled_launches(p, batch);
     if (grouped(p)) return hs_grouped_launches(p, batch);
     if (two_phase(p)) return hs_twophase_launches(p, batch);
     if (interleaved(p)) return hs_interleaved_launches(p, batch);
@@ -49,7 +49,8 @@ int hs_tiled_launches(const hs_plan *p, int64_t batch)
 
 int hs_launch_tiled(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
-    if (p->variant == HS_STANDARD) return hs_standard_tiled_launch(p, buf, batch, stream);
+    if (p->variant == HS_STANDARD)
+        return hs_standard_rb_supported(p) ? hs_standard_rb_launch(p, buf, batch, stream) : hs_standard_tiled_launch(p, buf, batch, stream);
     if (grouped(p)) return hs_grouped_launch(p, buf, batch, ws, stream);
     if (two_phase(p)) return hs_twophase_launch(p, buf, batch, ws, stream);
     if (interleaved(p)) return hs_interleaved_launch(p, buf, batch, ws, stream);
