@@ -60,9 +60,12 @@ enum hs_algo {
     HS_ALGO_TWOPHASE = 3, /* eqs. 2-3 only: the two-phase kernel (for eq. 2 the same as HS_ALGO_TILED)              */
     HS_ALGO_GATHER = 4,   /* eqs. 3-4 only: the range-skipping gather straight from x (no workspace); what
                              HS_ALGO_TILED itself uses for spectra too long for the interleaved group copy           */
-    HS_ALGO_GROUPED = 5   /* eqs. 2-3 only: two phases per spectrum by a static group of co-resident CTAs, the
+    HS_ALGO_GROUPED = 5,  /* eqs. 2-3 only: two phases per spectrum by a static group of co-resident CTAs, the
                              per-harmonic arrays of a spectrum live in one L2-resident workspace slot per group
-                             (cooperative launch); what HS_ALGO_TILED uses for eq. 2 when a slot fits L2            */
+                             (cooperative launch)                                                                   */
+    HS_ALGO_STREAMED = 6  /* eqs. 2-3, Hmax 16 or 32: two plain kernels (per-harmonic arrays of the large block sizes
+                             only, written to and read back from a workspace of one slot per spectrum; the small
+                             sizes are evaluated from the spectrum itself); any spectrum length                     */
 };
 
 /*

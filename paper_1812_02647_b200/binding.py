@@ -13,12 +13,12 @@ LIB_PATH = os.path.join(_HERE, "libhs.so")
 
 HS_STANDARD, HS_MAX, HS_FREQBIN, HS_GREEDY = 0, 1, 2, 3
 HS_OUT_FULL, HS_OUT_REDUCED, HS_OUT_BOTH = 1, 2, 3
-HS_ALGO_AUTO, HS_ALGO_DIRECT, HS_ALGO_TILED, HS_ALGO_TWOPHASE, HS_ALGO_GATHER, HS_ALGO_GROUPED = 0, 1, 2, 3, 4, 5
+HS_ALGO_AUTO, HS_ALGO_DIRECT, HS_ALGO_TILED, HS_ALGO_TWOPHASE, HS_ALGO_GATHER, HS_ALGO_GROUPED, HS_ALGO_STREAMED = 0, 1, 2, 3, 4, 5, 6
 HS_OK, HS_ERR_INVALID_ARG, HS_ERR_NULL_POINTER, HS_ERR_MISALIGNED, HS_ERR_UNSUPPORTED, HS_ERR_WORKSPACE, HS_ERR_CUDA = range(7)
 VARIANTS = {"standard": HS_STANDARD, "max": HS_MAX, "freqbin": HS_FREQBIN, "greedy": HS_GREEDY}
 OUT_MODES = {"full": HS_OUT_FULL, "reduced": HS_OUT_REDUCED, "both": HS_OUT_BOTH}
 ALGOS = {"auto": HS_ALGO_AUTO, "direct": HS_ALGO_DIRECT, "tiled": HS_ALGO_TILED, "twophase": HS_ALGO_TWOPHASE,
-         "gather": HS_ALGO_GATHER, "grouped": HS_ALGO_GROUPED}
+         "gather": HS_ALGO_GATHER, "grouped": HS_ALGO_GROUPED, "streamed": HS_ALGO_STREAMED}
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build the CUDA library with `python -m paper_1812_02647_b200.build` "

@@ -26,7 +26,7 @@ void resolve_algo(hs_plan *p)
 {
     if (p->algo_req == HS_ALGO_DIRECT) p->algo = HS_ALGO_DIRECT;
     else if (p->algo_req == HS_ALGO_TILED || p->algo_req == HS_ALGO_TWOPHASE || p->algo_req == HS_ALGO_GATHER ||
-             p->algo_req == HS_ALGO_GROUPED)
+             p->algo_req == HS_ALGO_GROUPED || p->algo_req == HS_ALGO_STREAMED)
         p->algo = HS_ALGO_TILED;
     else p->algo = hs_tiled_supported(p) ? HS_ALGO_TILED : HS_ALGO_DIRECT;
     p->ws = nullptr;
@@ -159,13 +159,15 @@ int hs_plan_algo(const hs_plan *p) { return p ? p->algo : -1; }
 int hs_plan_set_algo(hs_plan *p, int algo)
 {
     if (!p) HS_FAIL(HS_ERR_NULL_POINTER);
-    if (algo < HS_ALGO_AUTO || algo > HS_ALGO_GROUPED) HS_FAIL(HS_ERR_INVALID_ARG);
-    if ((algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GROUPED) && p->variant != HS_MAX && p->variant != HS_FREQBIN)
+    if (algo < HS_ALGO_AUTO || algo > HS_ALGO_STREAMED) HS_FAIL(HS_ERR_INVALID_ARG);
+    if ((algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GROUPED || algo == HS_ALGO_STREAMED) && p->variant != HS_MAX &&
+        p->variant != HS_FREQBIN)
         HS_FAIL(HS_ERR_INVALID_ARG);
     if (algo == HS_ALGO_GATHER && p->variant != HS_GREEDY && p->variant != HS_FREQBIN) HS_FAIL(HS_ERR_INVALID_ARG);
     const int before = p->algo_req;
     p->algo_req = algo;
-    if ((algo == HS_ALGO_TILED || algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GATHER || algo == HS_ALGO_GROUPED) &&
+    if ((algo == HS_ALGO_TILED || algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GATHER || algo == HS_ALGO_GROUPED ||
+         algo == HS_ALGO_STREAMED) &&
         !hs_tiled_supported(p)) {
         p->algo_req = before;
         HS_FAIL(HS_ERR_INVALID_ARG);

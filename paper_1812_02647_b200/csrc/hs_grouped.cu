@@ -26,6 +26,7 @@
 // A chunk owns the super-blocks (size j K_j, K_j the largest power of two with j K_j <= Hmax) that START inside it and
 // reads a 32-word halo for those that run past its end.
 #include <cstdlib>
+#include <utility>
 
 #include "hs_internal.cuh"
 #include "hs_ptx.cuh"
@@ -41,19 +42,30 @@ constexpr int kTab = kChunk + kHalo;      // table entries per width
 constexpr int kTileB = 128;               // phase-B outputs per warp tile (float4 per lane)
 constexpr size_t kL2Budget = (size_t)56 << 20;
 
+// Which per-harmonic arrays A_i exist.  HYB = 0 (grouped mode): every i = 2..Hmax.  HYB = 1 (streamed mode, below): the
+// small sizes are evaluated by phase B straight from the spectrum (a window of i words per output costs as much HBM
+// traffic as writing and re-reading A_i while i is small), so Max keeps only i not in {2, 3, 4, 6, 8} and freq-bin only i > 8.
+__host__ __device__ constexpr bool stored(int variant, int hyb, int i)
+{
+    if (!hyb) return true;
+    if (variant == HS_MAX) return !(i == 2 || i == 3 || i == 4 || i == 6 || i == 8);
+    return i > 8;
+}
+
 struct gr_layout {
     int off[33];  // word offset of A_i inside a slot (multiple of 32: 128-byte rows), i = 2..Hmax
     int len[33];  // ceil(N / i): entries of A_i that can be non-zero
     int64_t slot_words;
 };
 
-gr_layout make_layout(int N, int Hmax)
+gr_layout make_layout(int N, int Hmax, int variant = HS_MAX, int hyb = 0)
 {
     gr_layout lay{};
     int64_t o = 0;
     for (int i = 2; i <= Hmax; i++) {
         lay.off[i] = (int)o;
         lay.len[i] = (N + i - 1) / i;
+        if (!stored(variant, hyb, i)) continue;
         o += (lay.len[i] + 8 + 31) & ~31;  // padded: vector stores/loads at any n < len stay inside the row
     }
     lay.slot_words = (o + 63) & ~(int64_t)63;
@@ -157,8 +169,8 @@ __device__ __forceinline__ void max_tables(const gr_smem &sm)
 }
 
 // Max: the power-of-two block sizes from the thread's 8 aligned raw words (sizes 16 and 32 by shuffles).
-template <int HMAX>
-__device__ __forceinline__ void max_pow2(const gr_params &p, const gr_smem &sm, unsigned s0, int k0)
+template <int HMAX, int HYB>
+__device__ __forceinline__ void max_pow2(const gr_params &p, const gr_smem &sm, float *__restrict__ Ab, int k0)
 {
     const int lane = threadIdx.x & 31;
 #pragma unroll
@@ -173,23 +185,25 @@ __device__ __forceinline__ void max_pow2(const gr_params &p, const gr_smem &sm, 
     const float e32 = fmaxf(e16, __shfl_xor_sync(0xffffffffu, e16, 2));
     if (k >= p.N) continue;
     const bool whole = k + 8 <= p.N;                          // else exactly 4 bins are left (N % 4 == 0)
-    float *A2 = p.A + (s0 + (unsigned)p.lay.off[2] + (unsigned)(k >> 1));
-    if (whole) *reinterpret_cast<float4 *>(A2) = make_float4(m0, m1, m2, m3);
-    else *reinterpret_cast<float2 *>(A2) = make_float2(m0, m1);
-    if (HMAX >= 4) {
-        float *A4 = p.A + (s0 + (unsigned)p.lay.off[4] + (unsigned)(k >> 2));
-        if (whole) *reinterpret_cast<float2 *>(A4) = make_float2(q0, q1);
-        else A4[0] = q0;
+    if (!HYB) {
+        float *A2 = Ab + ((unsigned)p.lay.off[2] + (unsigned)(k >> 1));
+        if (whole) *reinterpret_cast<float4 *>(A2) = make_float4(m0, m1, m2, m3);
+        else *reinterpret_cast<float2 *>(A2) = make_float2(m0, m1);
+        if (HMAX >= 4) {
+            float *A4 = Ab + ((unsigned)p.lay.off[4] + (unsigned)(k >> 2));
+            if (whole) *reinterpret_cast<float2 *>(A4) = make_float2(q0, q1);
+            else A4[0] = q0;
+        }
+        if (HMAX >= 8) Ab[(unsigned)p.lay.off[8] + (unsigned)(k >> 3)] = e8;
     }
-    if (HMAX >= 8) p.A[s0 + (unsigned)p.lay.off[8] + (unsigned)(k >> 3)] = e8;
-    if (HMAX >= 16 && (lane & 1) == 0) p.A[s0 + (unsigned)p.lay.off[16] + (unsigned)(k >> 4)] = e16;
-    if (HMAX >= 32 && (lane & 3) == 0) p.A[s0 + (unsigned)p.lay.off[32] + (unsigned)(k >> 5)] = e32;
+    if (HMAX >= 16 && (lane & 1) == 0) Ab[(unsigned)p.lay.off[16] + (unsigned)(k >> 4)] = e16;
+    if (HMAX >= 32 && (lane & 3) == 0) Ab[(unsigned)p.lay.off[32] + (unsigned)(k >> 5)] = e32;
     }
 }
 
 // freq-bin: the power-of-two decimations straight from the raw words.
-template <int HMAX>
-__device__ __forceinline__ void dec_pow2(const gr_params &p, const gr_smem &sm, unsigned s0, int k0)
+template <int HMAX, int HYB>
+__device__ __forceinline__ void dec_pow2(const gr_params &p, const gr_smem &sm, float *__restrict__ Ab, int k0)
 {
     const int lane = threadIdx.x & 31;
 #pragma unroll
@@ -199,28 +213,32 @@ __device__ __forceinline__ void dec_pow2(const gr_params &p, const gr_smem &sm, 
     const float4 u = *reinterpret_cast<const float4 *>(sm.raw + p0);
     const float4 w = *reinterpret_cast<const float4 *>(sm.raw + p0 + 4);
     const bool whole = k + 8 <= p.N;
-    float *A2 = p.A + (s0 + (unsigned)p.lay.off[2] + (unsigned)(k >> 1));
-    if (whole) *reinterpret_cast<float4 *>(A2) = make_float4(u.x, u.z, w.x, w.z);
-    else *reinterpret_cast<float2 *>(A2) = make_float2(u.x, u.z);
-    if (HMAX >= 4) {
-        float *A4 = p.A + (s0 + (unsigned)p.lay.off[4] + (unsigned)(k >> 2));
-        if (whole) *reinterpret_cast<float2 *>(A4) = make_float2(u.x, w.x);
-        else A4[0] = u.x;
+    if (!HYB) {
+        float *A2 = Ab + ((unsigned)p.lay.off[2] + (unsigned)(k >> 1));
+        if (whole) *reinterpret_cast<float4 *>(A2) = make_float4(u.x, u.z, w.x, w.z);
+        else *reinterpret_cast<float2 *>(A2) = make_float2(u.x, u.z);
+        if (HMAX >= 4) {
+            float *A4 = Ab + ((unsigned)p.lay.off[4] + (unsigned)(k >> 2));
+            if (whole) *reinterpret_cast<float2 *>(A4) = make_float2(u.x, w.x);
+            else A4[0] = u.x;
+        }
+        if (HMAX >= 8) Ab[(unsigned)p.lay.off[8] + (unsigned)(k >> 3)] = u.x;
     }
-    if (HMAX >= 8) p.A[s0 + (unsigned)p.lay.off[8] + (unsigned)(k >> 3)] = u.x;
-    if (HMAX >= 16 && (lane & 1) == 0) p.A[s0 + (unsigned)p.lay.off[16] + (unsigned)(k >> 4)] = u.x;
-    if (HMAX >= 32 && (lane & 3) == 0) p.A[s0 + (unsigned)p.lay.off[32] + (unsigned)(k >> 5)] = u.x;
+    if (HMAX >= 16 && (lane & 1) == 0) Ab[(unsigned)p.lay.off[16] + (unsigned)(k >> 4)] = u.x;
+    if (HMAX >= 32 && (lane & 3) == 0) Ab[(unsigned)p.lay.off[32] + (unsigned)(k >> 5)] = u.x;
     }
 }
 
 // store the CNT entries of size JD held in m[0..CNT) for super-block q, then halve (pairwise maxima) and recurse
-template <int JD, int CNT, int DUMMY>
-__device__ __forceinline__ void direct_levels(const gr_params &p, unsigned s0, int q, float *m)
+template <int JD, int CNT, int HYB>
+__device__ __forceinline__ void direct_levels(const gr_params &p, float *__restrict__ Ab, int q, float *m)
 {
     const int n0 = CNT * q;
     const int len = p.lay.len[JD];
-    float *__restrict__ g = p.A + (s0 + (unsigned)p.lay.off[JD] + (unsigned)n0);
-    if (n0 + CNT <= len) {
+    float *__restrict__ g = Ab + ((unsigned)p.lay.off[JD] + (unsigned)n0);
+    if constexpr (!stored(HS_MAX, HYB, JD)) {                                 // (size JD is not kept: phase B reads the spectrum)
+        (void)len, (void)g;
+    } else if (n0 + CNT <= len) {
         if constexpr (CNT == 8) {
             *reinterpret_cast<float4 *>(g) = make_float4(m[0], m[1], m[2], m[3]);
             *reinterpret_cast<float4 *>(g + 4) = make_float4(m[4], m[5], m[6], m[7]);
@@ -239,15 +257,15 @@ __device__ __forceinline__ void direct_levels(const gr_params &p, unsigned s0, i
     if constexpr (CNT > 1) {
 #pragma unroll
         for (int k = 0; k < CNT / 2; k++) m[k] = fmaxf(m[2 * k], m[2 * k + 1]);
-        direct_levels<JD * 2, CNT / 2, DUMMY>(p, s0, q, m);
+        direct_levels<JD * 2, CNT / 2, HYB>(p, Ab, q, m);
     }
 }
 
 // ---- odd sizes J = 3, 5, .., and their doublings 2J, 4J, .. <= HMAX ------------------------------------------------
 // Max, J < 8: one thread reduces one whole super-block (J K words, K = chain_len) held in registers: K maxima of
 // size J, then the pairwise pyramid, stored as vectors.  No table needed, ~1.6 instructions per input word.
-template <int J, int HMAX, int W0>
-__device__ __forceinline__ void max_direct(const gr_params &p, const gr_smem &sm, unsigned s0, int k0)
+template <int J, int HMAX, int W0, int HYB>
+__device__ __forceinline__ void max_direct(const gr_params &p, const gr_smem &sm, float *__restrict__ Ab, int k0)
 {
     constexpr int K = chain_len(J, HMAX), D = ilog2c(K), SB = J * K;
     constexpr int VW = SB % 4 == 0 ? 4 : SB % 2 == 0 ? 2 : 1;             // widest aligned shared-memory load
@@ -280,7 +298,7 @@ __device__ __forceinline__ void max_direct(const gr_params &p, const gr_smem &sm
 #pragma unroll
         for (int t = 1; t < J; t++) m[k] = fmaxf(m[k], v[J * k + t]);
     }
-    direct_levels<J, K, 0>(p, s0, q, m);
+    direct_levels<J, K, HYB>(p, Ab, q, m);
     }
 }
 
@@ -301,7 +319,7 @@ __device__ __forceinline__ void stg_lt(int n, int lim, float *base, unsigned idx
 // base + immediate.  freq-bin: A_I[n] = raw[I n - k0] (any I that is not a power of two).  Max: odd I >= 9, the block
 // maximum from two table entries, and for 2 I <= HMAX the maximum of the lane pair as A_2I[n / 2].
 template <int VARIANT, int I, int HMAX, int W0, int NW>
-__device__ __forceinline__ void row_pass(const gr_params &p, const gr_smem &sm, unsigned s0, int k0)
+__device__ __forceinline__ void row_pass(const gr_params &p, const gr_smem &sm, float *__restrict__ Ab, int k0)
 {
     constexpr int K = VARIANT == HS_MAX ? chain_len(I, HMAX) : 1;
     static_assert(K <= 2, "row_pass handles at most one doubling");
@@ -313,12 +331,12 @@ __device__ __forceinline__ void row_pass(const gr_params &p, const gr_smem &sm, 
     const int2 bd = sm.bounds[I];                                         // entries [bd.x, bd.y) belong to the chunk
     const int n = bd.x + 32 * wq + lane;
     const float *__restrict__ s = (W == 1 ? sm.raw : W == 8 ? sm.T8 : sm.T16) + (I * n - k0);
-    const unsigned g1 = s0 + (unsigned)p.lay.off[I] + (unsigned)n;
+    const unsigned g1 = (unsigned)p.lay.off[I] + (unsigned)n;
     const int lim1 = min(bd.y, p.lay.len[I]);
     unsigned g2 = 0;
     int lim2 = 0;
     if (K == 2) {
-        g2 = s0 + (unsigned)p.lay.off[2 * I <= 32 ? 2 * I : 32] + (unsigned)(n >> 1);
+        g2 = (unsigned)p.lay.off[2 * I <= 32 ? 2 * I : 32] + (unsigned)(n >> 1);
         lim2 = (lane & 1) ? 0 : min(bd.y, 2 * p.lay.len[2 * I <= 32 ? 2 * I : 32]);
     }
 #pragma unroll
@@ -333,10 +351,10 @@ __device__ __forceinline__ void row_pass(const gr_params &p, const gr_smem &sm, 
         switch (t) {   // (the byte offset must be an immediate)
 #define HS_ROW_CASE(T)                                                                        \
     case T:                                                                                   \
-        stg_lt<4 * 32 * NW * T>(nt, lim1, p.A, g1, v);                                        \
+        stg_lt<4 * 32 * NW * T>(nt, lim1, Ab, g1, v);                                        \
         if (K == 2) {                                                                         \
             const float w = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));                     \
-            stg_lt<4 * 16 * NW * T>(nt, lim2, p.A, g2, w);                                    \
+            stg_lt<4 * 16 * NW * T>(nt, lim2, Ab, g2, w);                                    \
         }                                                                                     \
         break;
             HS_ROW_CASE(0) HS_ROW_CASE(1) HS_ROW_CASE(2) HS_ROW_CASE(3) HS_ROW_CASE(4) HS_ROW_CASE(5) HS_ROW_CASE(6)
@@ -368,14 +386,14 @@ constexpr int w0_of(int variant, int I, int hmax)
     return w % kWarps;
 }
 
-template <int VARIANT, int HMAX, int I = 3>
-__device__ __forceinline__ void other_sizes(const gr_params &p, const gr_smem &sm, unsigned s0, int k0)
+template <int VARIANT, int HMAX, int HYB, int I = 3>
+__device__ __forceinline__ void other_sizes(const gr_params &p, const gr_smem &sm, float *__restrict__ Ab, int k0)
 {
     if constexpr (I <= HMAX) {
         constexpr int W0 = w0_of(VARIANT, I, HMAX), NW = nw_of(VARIANT, I, HMAX);
-        if constexpr (is_direct(VARIANT, I)) max_direct<I, HMAX, W0>(p, sm, s0, k0);
-        else if constexpr (is_row(VARIANT, I)) row_pass<VARIANT, I, HMAX, W0, NW>(p, sm, s0, k0);
-        other_sizes<VARIANT, HMAX, I + 1>(p, sm, s0, k0);
+        if constexpr (is_direct(VARIANT, I)) max_direct<I, HMAX, W0, HYB>(p, sm, Ab, k0);
+        else if constexpr (is_row(VARIANT, I) && stored(VARIANT, HYB, I)) row_pass<VARIANT, I, HMAX, W0, NW>(p, sm, Ab, k0);
+        other_sizes<VARIANT, HMAX, HYB, I + 1>(p, sm, Ab, k0);
     }
 }
 
@@ -412,31 +430,31 @@ __device__ __forceinline__ void emit_upper(const gr_params &p, const gr_smem &sm
 }
 
 // all A_i segments owned by the chunk at k0 (raw is complete and zero padded; bounds are set)
-template <int VARIANT, int HMAX>
-__device__ __forceinline__ void phaseA_chunk(const gr_params &p, const gr_smem &sm, unsigned s0, int k0)
+template <int VARIANT, int HMAX, int HYB>
+__device__ __forceinline__ void phaseA_chunk(const gr_params &p, const gr_smem &sm, float *__restrict__ Ab, int k0)
 {
     if (VARIANT == HS_MAX) {
         if (HMAX >= 16) max_tables<HMAX>(sm);
-        max_pow2<HMAX>(p, sm, s0, k0);
+        max_pow2<HMAX, HYB>(p, sm, Ab, k0);
         if (HMAX >= 16) __syncthreads();                       // tables complete
     } else {
-        dec_pow2<HMAX>(p, sm, s0, k0);
+        dec_pow2<HMAX, HYB>(p, sm, Ab, k0);
     }
-    other_sizes<VARIANT, HMAX>(p, sm, s0, k0);
+    other_sizes<VARIANT, HMAX, HYB>(p, sm, Ab, k0);
 }
 
 // ---------------------------------------------------------------------------------------------- phase B
 // One warp tile = 128 consecutive outputs below n_split: lane holds bins n_first + 4 lane .. +3 as one float4.
 // The loads of a level are issued in batches of up to 8 float4 before they are consumed (memory-level parallelism).
 template <int L, int OUT>
-__device__ __forceinline__ void phaseB_tile(const gr_params &p, unsigned s0, int64_t row, int n_first)
+__device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__restrict__ Ab, int64_t row, int n_first)
 {
     const int N = p.N;
     const int n = n_first + 4 * (threadIdx.x & 31);
     const bool live = n < N;                                       // (N % 4 == 0: a float4 is wholly inside or outside)
     float4 S = live ? __ldg(reinterpret_cast<const float4 *>(p.x + row + n)) : make_float4(0.f, 0.f, 0.f, 0.f);
     hs_emit<OUT> e0, e1, e2, e3;
-    const float *__restrict__ An = p.A + (s0 + (unsigned)n);       // A_i[n] = An[off_i]
+    const float *__restrict__ An = Ab + ((unsigned)n);       // A_i[n] = An[off_i]
     auto emit = [&](int l) {
         const float c = hs_norm(l);
         const float4 h = make_float4(S.x * c, S.y * c, S.z * c, S.w * c);
@@ -526,7 +544,7 @@ gr_kernel(const __grid_constant__ gr_params p)
     sm.T8 = dyn + kRawBufs * kRaw;
     sm.T16 = sm.T8 + (kTables && HMAX >= 32 ? kTab : 0);
     sm.bounds = s_bounds;
-    const unsigned s0 = (unsigned)grp * (unsigned)p.lay.slot_words;   // word offset of the group's slot (< 2^32: checked on the host)
+    float *__restrict__ Ab = p.A + (int64_t)grp * p.lay.slot_words;   // the group's slot
     int *cntA = p.ctrl + 32 + 64 * grp, *cntB = cntA + 32;
 
     if (threadIdx.x == 0) {
@@ -593,7 +611,7 @@ gr_kernel(const __grid_constant__ gr_params p)
             const int valid = min(kChunk + kHalo, N - k0);                // words the copy delivered (multiple of 4)
             for (int w = valid + threadIdx.x; w < kRaw; w += kThreads) sm.raw[w] = 0.0f;   // zero padding (C5)
             __syncthreads();
-            if (!(p.dbg & 1)) phaseA_chunk<VARIANT, HMAX>(p, sm, s0, k0);
+            if (!(p.dbg & 1)) phaseA_chunk<VARIANT, HMAX, 0>(p, sm, Ab, k0);
             if (k0 >= p.n_split) emit_upper<L, OUT>(p, sm, (int64_t)b * N, k0);
             __syncthreads();                                              // raw/tables/bounds are reused
             tick(2);
@@ -616,7 +634,7 @@ gr_kernel(const __grid_constant__ gr_params p)
             j = __shfl_sync(0xffffffffu, j, 0);
             const int tile = rank + p.GS * j;
             if (tile >= p.ntiles || (p.dbg & 2)) break;
-            phaseB_tile<L, OUT>(p, s0, row, tile * kTileB);
+            phaseB_tile<L, OUT>(p, Ab, row, tile * kTileB);
         }
         __syncthreads();                                                  // every load of the slot has returned
         tick(4);
@@ -726,6 +744,236 @@ int by_hmax(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cu
     }
 }
 
+
+// ====================================================================================================================
+// Streamed mode (HS_ALGO_STREAMED): the same two phases as two PLAIN kernels per wave of spectra, no inter-CTA
+// synchronisation at all.  Phase A (one CTA per 4096-word chunk, the code above with HYB = 1) keeps only the arrays
+// phase B cannot get cheaply from the spectrum itself; phase B (one thread per output bin below n_split) evaluates the
+// small block sizes / strides straight from x -- a window of i consecutive words per output, read with the widest
+// aligned vector load -- and adds the kept A_i with unit stride.  Per bin at Hmax = 32 the kept arrays are 1.68 (Max)
+// or 1.34 (freq-bin) words instead of 3.06, and every kernel is a plain stream over its inputs, so the mode works for
+// any spectrum length and is bound by HBM (x twice, the kept arrays written and read once, the outputs once:
+// 26.4 B/bin for Max) when a wave's arrays do not fit L2, and by L2 when they do (wave = HS_ST_WAVE spectra).
+constexpr bool st_hmax_ok(int hmax) { return hmax == 16 || hmax == 32; }
+
+template <int VARIANT, int HMAX, int OUT>
+__global__ void __launch_bounds__(kThreads, 4)
+st_phaseA_kernel(const __grid_constant__ gr_params p, int b0)
+{
+    constexpr int L = ilog2c(HMAX) + 1;
+    constexpr bool kTables = VARIANT == HS_MAX && HMAX >= 16;
+    extern __shared__ __align__(128) float dyn[];
+    __shared__ __align__(8) uint64_t bar;
+    __shared__ int2 s_bounds[33];
+    const int b = b0 + blockIdx.y, k0 = blockIdx.x * kChunk, N = p.N;
+    gr_smem sm;
+    sm.raw = dyn;
+    sm.T8 = dyn + kRaw;
+    sm.T16 = sm.T8 + (kTables && HMAX >= 32 ? kTab : 0);
+    sm.bounds = s_bounds;
+    const int valid = min(kChunk + kHalo, N - k0);                       // words of the spectrum in chunk + halo (multiple of 4)
+    if (threadIdx.x == 0) {
+        hsptx::mbar_init(&bar, 1);
+        hsptx::mbar_fence_init();
+        hsptx::mbar_arrive_expect_tx(&bar, (uint32_t)valid * 4u);
+        hsptx::bulk_g2s(dyn, p.x + (int64_t)b * N + k0, (uint32_t)valid * 4u, &bar);
+    }
+    if (threadIdx.x >= 3 && threadIdx.x <= HMAX) {
+        // entries of size i owned by the chunk: those whose super-block (i K words) starts inside it
+        const int i = threadIdx.x, K = VARIANT == HS_MAX ? chain_len(i, HMAX) : 1, sb = i * K;
+        const int first = K * ((k0 + sb - 1) / sb), last = K * ((k0 + kChunk + sb - 1) / sb);
+        const int lenK = (p.lay.len[i] + K - 1) / K * K;
+        s_bounds[i] = make_int2(first, min(last, lenK));
+    }
+    for (int w = valid + threadIdx.x; w < kRaw; w += kThreads) dyn[w] = 0.0f;   // zero padding (C5); disjoint from the copy
+    __syncthreads();                                                       // barrier initialised, bounds and padding visible
+    hsptx::mbar_wait(&bar, 0u);
+    float *__restrict__ Ab = p.A + (int64_t)(b % p.groups) * p.lay.slot_words;
+    phaseA_chunk<VARIANT, HMAX, 1>(p, sm, Ab, k0);
+    if (k0 >= p.n_split) emit_upper<L, OUT>(p, sm, (int64_t)b * N, k0);
+}
+
+// term of harmonic I at bin n, every element in range: the maximum of x[I n .. I n + I - 1] (Max) or x[I n] (freq-bin)
+template <int VARIANT, int I>
+__device__ __forceinline__ float st_term_safe(const float *__restrict__ xb, int n)
+{
+    const float *__restrict__ w = xb + (int64_t)I * n;
+    if (VARIANT == HS_FREQBIN) return __ldg(w);
+    if constexpr (I % 4 == 0) {
+        float m = 0.f;
+#pragma unroll
+        for (int q = 0; q < I / 4; q++) {
+            const float4 u = __ldg(reinterpret_cast<const float4 *>(w) + q);
+            const float t = fmaxf(fmaxf(u.x, u.y), fmaxf(u.z, u.w));
+            m = q == 0 ? t : fmaxf(m, t);
+        }
+        return m;
+    } else if constexpr (I % 2 == 0) {
+        float m = 0.f;
+#pragma unroll
+        for (int q = 0; q < I / 2; q++) {
+            const float2 u = __ldg(reinterpret_cast<const float2 *>(w) + q);
+            const float t = fmaxf(u.x, u.y);
+            m = q == 0 ? t : fmaxf(m, t);
+        }
+        return m;
+    } else {
+        float m = __ldg(w);
+#pragma unroll
+        for (int q = 1; q < I; q++) m = fmaxf(m, __ldg(w + q));
+        return m;
+    }
+}
+// the same with zero padding beyond the spectrum (C5: the zeros take part in the maximum)
+template <int VARIANT, int I>
+__device__ __forceinline__ float st_term_edge(const float *__restrict__ xb, int n, int N)
+{
+    const int k = I * n;
+    if (VARIANT == HS_FREQBIN) return k < N ? __ldg(xb + k) : 0.f;
+    float m = k < N ? __ldg(xb + k) : 0.f;
+#pragma unroll
+    for (int q = 1; q < I; q++) m = fmaxf(m, k + q < N ? __ldg(xb + k + q) : 0.f);
+    return m;
+}
+
+constexpr int kStThreads = 256;
+
+template <class F, int... k>
+__device__ __forceinline__ void st_static_for(F &f, std::integer_sequence<int, k...>)
+{
+    (f(std::integral_constant<int, k>{}), ...);
+}
+
+template <int VARIANT, int HMAX, int OUT>
+__global__ void __launch_bounds__(kStThreads)
+st_phaseB_kernel(const __grid_constant__ gr_params p, int b0)
+{
+    constexpr int L = ilog2c(HMAX) + 1;
+    const int N = p.N, b = b0 + blockIdx.y;
+    const int n_end = min(N, p.n_split);                               // bins [n_end, N) were emitted by phase A
+    const int n = blockIdx.x * kStThreads + threadIdx.x;
+    const int n_lo = n & ~31;                                          // first bin of the warp
+    if (n_lo >= n_end) return;
+    const bool live = n < n_end;
+    const int nn = live ? n : n_end - 1;                               // lanes past the end shadow the last bin, store nothing
+    const int n_hi1 = min(n_lo + 32, n_end);                           // one past the warp's last bin
+    const float *__restrict__ xb = p.x + (int64_t)b * N;
+    const float *__restrict__ An = p.A + (int64_t)(b % p.groups) * p.lay.slot_words + nn;   // A_i[n] = An[off_i]
+    float S = __ldg(xb + nn);
+    hs_emit<OUT> e;
+    float *plane0 = (OUT & HS_OUT_FULL) ? p.sums + ((int64_t)b * L * N + nn) : nullptr;
+    auto emit = [&](int l) {
+        const float h = S * hs_norm(l);
+        if ((OUT & HS_OUT_FULL) && live) hsptx::st_cs(plane0 + (int64_t)l * N, h);
+        if (OUT & HS_OUT_REDUCED) e.reduce(l, h);
+    };
+    emit(0);
+    bool tail = false;
+    auto level = [&](auto lc) {
+        constexpr int l = decltype(lc)::value + 1, lo = (1 << (l - 1)) + 1, hi = 1 << l;
+        if ((int64_t)lo * n_lo < N) {                                  // warp-uniform: the level has a harmonic in range
+            auto harmonic = [&](auto ic) {
+                constexpr int i = decltype(ic)::value + lo;
+                if ((int64_t)i * n_hi1 <= N) {                         // warp-uniform: in range for every lane
+                    if constexpr (stored(VARIANT, 1, i)) S += __ldg(An + p.lay.off[i]);
+                    else S += st_term_safe<VARIANT, i>(xb, nn);
+                } else if ((int64_t)i * n_lo < N) {                    // warp-uniform: in range for some lane
+                    if constexpr (stored(VARIANT, 1, i)) S += nn < p.lay.len[i] ? __ldg(An + p.lay.off[i]) : 0.f;
+                    else S += st_term_edge<VARIANT, i>(xb, nn, N);
+                }
+            };
+            st_static_for(harmonic, std::make_integer_sequence<int, hi - lo + 1>{});
+            emit(l);
+        } else if (OUT != HS_OUT_REDUCED) {
+            emit(l);
+        } else {
+            tail = true;
+        }
+    };
+    st_static_for(level, std::make_integer_sequence<int, L - 1>{});
+    // With S unchanged over the skipped levels h_l = S c_l is monotone in l: testing the last level alone is enough.
+    if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
+    if ((OUT & HS_OUT_REDUCED) && live) {
+        hsptx::st_cs(p.vmax + (int64_t)b * N + n, e.m);
+        hsptx::st_cs(p.amax + (int64_t)b * N + n, (uint8_t)e.a);
+    }
+}
+
+struct st_sched {
+    gr_layout lay;
+    int64_t wave, slots;   // spectra per wave, workspace slots
+    int nchunks, n_split;
+};
+
+st_sched st_make_sched(const hs_plan *p, int64_t batch)
+{
+    st_sched s{};
+    const int N = (int)p->nbins;
+    s.lay = make_layout(N, p->Hmax, p->variant, 1);
+    s.nchunks = (N + kChunk - 1) / kChunk;
+    s.n_split = (int)(((int64_t)(N + 1) / 2 + kChunk - 1) / kChunk * kChunk);
+    int64_t wave = batch < 32768 ? batch : 32768;                       // gridDim.y
+    if (getenv("HS_ST_WAVE")) wave = atoi(getenv("HS_ST_WAVE"));
+    if (wave < 1) wave = 1;
+    if (wave > batch) wave = batch;
+    if (wave > 32768) wave = 32768;
+    s.wave = wave;
+    s.slots = wave;
+    return s;
+}
+
+template <int VARIANT, int HMAX, int OUT>
+int st_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    const st_sched s = st_make_sched(p, batch);
+    gr_params prm{};
+    prm.x = buf.x;
+    prm.A = static_cast<float *>(ws);
+    prm.sums = buf.sums;
+    prm.vmax = buf.vmax;
+    prm.amax = buf.amax;
+    prm.lay = s.lay;
+    prm.N = (int)p->nbins;
+    prm.B = (int)batch;
+    prm.groups = (int)s.slots;
+    prm.nchunks = s.nchunks;
+    prm.n_split = s.n_split;
+    auto kA = st_phaseA_kernel<VARIANT, HMAX, OUT>;
+    auto kB = st_phaseB_kernel<VARIANT, HMAX, OUT>;
+    const size_t smem = smem_bytes(VARIANT, HMAX) + (VARIANT == HS_MAX ? 0 : 0);
+    static bool configured = false;
+    if (!configured) {
+        HS_CUDA_OK(cudaFuncSetAttribute(kA, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured = true;
+    }
+    const int n_end = s.n_split < prm.N ? s.n_split : prm.N;
+    const unsigned tilesB = (unsigned)((n_end + kStThreads - 1) / kStThreads);
+    for (int64_t b0 = 0; b0 < batch; b0 += s.wave) {
+        const unsigned nb = (unsigned)(batch - b0 < s.wave ? batch - b0 : s.wave);
+        kA<<<dim3((unsigned)s.nchunks, nb), kThreads, smem, stream>>>(prm, (int)b0);
+        kB<<<dim3(tilesB, nb), kStThreads, 0, stream>>>(prm, (int)b0);
+    }
+    HS_CUDA_OK(cudaGetLastError());
+    return HS_OK;
+}
+
+template <int VARIANT, int HMAX>
+int st_by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    switch (p->out_mode) {
+        case HS_OUT_FULL: return st_launch<VARIANT, HMAX, HS_OUT_FULL>(p, buf, batch, ws, stream);
+        case HS_OUT_REDUCED: return st_launch<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
+        default: return st_launch<VARIANT, HMAX, HS_OUT_BOTH>(p, buf, batch, ws, stream);
+    }
+}
+
+template <int VARIANT>
+int st_by_hmax(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    if (p->Hmax == 16) return st_by_out<VARIANT, 16>(p, buf, batch, ws, stream);
+    return st_by_out<VARIANT, 32>(p, buf, batch, ws, stream);
+}
+
 }  // namespace
 
 // One slot per group must fit the L2 budget: spectra of up to ~2^22 bins; Hmax = 1 has no phase A at all.
@@ -755,4 +1003,31 @@ int hs_grouped_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, vo
     if (!ws) HS_FAIL(HS_ERR_WORKSPACE);
     if (p->variant == HS_FREQBIN) return by_hmax<HS_FREQBIN>(p, buf, batch, ws, stream);
     return by_hmax<HS_MAX>(p, buf, batch, ws, stream);
+}
+
+// ---- streamed mode
+bool hs_streamed_supported(const hs_plan *p)
+{
+    if (p->variant != HS_MAX && p->variant != HS_FREQBIN) return false;
+    if (!st_hmax_ok(p->Hmax)) return false;
+    return p->nbins * 4 + 64 < ((int64_t)1 << 31);                     // word offsets inside a slot are 32-bit
+}
+
+size_t hs_streamed_workspace_bytes(const hs_plan *p, int64_t batch)
+{
+    const st_sched s = st_make_sched(p, batch);
+    return (size_t)s.slots * (size_t)s.lay.slot_words * 4 + 256;
+}
+
+int hs_streamed_launches(const hs_plan *p, int64_t batch)
+{
+    const st_sched s = st_make_sched(p, batch);
+    return (int)(2 * ((batch + s.wave - 1) / s.wave));
+}
+
+int hs_streamed_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    if (!ws) HS_FAIL(HS_ERR_WORKSPACE);
+    if (p->variant == HS_FREQBIN) return st_by_hmax<HS_FREQBIN>(p, buf, batch, ws, stream);
+    return st_by_hmax<HS_MAX>(p, buf, batch, ws, stream);
 }

@@ -25,6 +25,8 @@
 // serial dependence j -> address -> load, and the outputs of a thread are two float4 and two 4-byte stores.  Range
 // handling is warp-uniform (a warp owns 16 consecutive bins): harmonic i is in range for every lane iff
 // i (n_hi + 1) <= N.
+#include <cstdlib>
+
 #include "hs_internal.cuh"
 #include "hs_ptx.cuh"
 
@@ -37,7 +39,7 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kWarpBins = 8 * C;                        // 32 bins per warp
 constexpr int kGTile = kWarps * kWarpBins;              // 256 bins per gather tile
 constexpr int kGSub = 2;                                // tiles per G item above the heavy region (bins >= N/8), 1 below
-constexpr int kLag = 2;                                 // the gather runs kLag steps behind the copy
+constexpr int kLagDefault = 2;                          // the gather runs `lag` steps behind the copy
 constexpr int kTBins = 512;                             // bins per T item
 constexpr int kTStride = kTBins + 4;                    // shared-memory row stride (floats) of the copy tile
 constexpr int kMaxRing = 4;
@@ -50,7 +52,7 @@ struct il_params {
     uint8_t *amax;
     int *ctrl;          // [0] work counter, [1] error flag, [2..5] wait statistics, [16 + g] T items done, [16 + groups + g] G items done
     int64_t slot_words;
-    int N, B, groups, R;
+    int N, B, groups, R, lag;
     int nT, nG;         // items per group
     int nHeavy;         // the first nHeavy G items are single tiles (bins below ~N/8: 8 to 32 harmonics per bin)
     int n_split;        // G items cover bins [0, n_split); T items emit the outputs of [n_split, N)
@@ -313,7 +315,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
     int *queue = p.ctrl, *err = p.ctrl + 1;
     int *doneT = p.ctrl + 16, *doneG = p.ctrl + 16 + p.groups;
     const int per = p.nT + p.nG;
-    const int total = (p.groups + kLag) * per;
+    const int total = (p.groups + p.lag) * per;
     int lastT = -1, lastG = -1;                                         // thread 0: groups already seen complete
     if (threadIdx.x == 0) s_item = atomicAdd(queue, 1);
     __syncthreads();
@@ -339,8 +341,8 @@ il_persistent_kernel(const __grid_constant__ il_params p)
                     atomicAdd(doneT + s, 1);
                 }
             }
-        } else if (s >= kLag) {                                         // ---- G item (r - t_before) of group s - kLag
-            const int grp = s - kLag;
+        } else if (s >= p.lag) {                                         // ---- G item (r - t_before) of group s - kLag
+            const int grp = s - p.lag;
             const float *xT = p.xT + (int64_t)(grp % p.R) * p.slot_words;
             if (threadIdx.x == 0 && lastT < grp) {
                 wait_count(doneT + grp, p.nT, err, p.ctrl + 4);
@@ -369,7 +371,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
 }
 
 struct il_sched {
-    int groups, R, nT, nG, nHeavy, n_split;
+    int groups, R, lag, nT, nG, nHeavy, n_split;
     int64_t slot_words;
 };
 
@@ -378,7 +380,11 @@ il_sched make_sched(const hs_plan *p, int64_t batch)
     il_sched s{};
     const int N = (int)p->nbins;
     s.groups = (int)((batch + G - 1) / G);
-    s.R = s.groups < kMaxRing ? s.groups : kMaxRing;
+    int ring = kMaxRing;
+    s.lag = kLagDefault;
+    if (getenv("HS_IL_RING")) ring = atoi(getenv("HS_IL_RING"));
+    if (getenv("HS_IL_LAG")) s.lag = atoi(getenv("HS_IL_LAG"));
+    s.R = s.groups < ring ? s.groups : ring;
     s.nT = (N + kTBins - 1) / kTBins;
     // bins n >= N/2 have S_H(n) = x(n): the T items emit them.  The split is a multiple of the T tile.
     const int half = (N + 1) / 2;
@@ -412,6 +418,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.B = (int)batch;
     prm.groups = s.groups;
     prm.R = s.R;
+    prm.lag = s.lag;
     prm.nT = s.nT;
     prm.nG = s.nG;
     prm.nHeavy = s.nHeavy;
@@ -424,7 +431,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
         ctas_per_sm = occ > 0 ? occ : 1;
     }
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(s.groups), stream));
-    const int64_t total = (int64_t)(s.groups + kLag) * (s.nT + s.nG);
+    const int64_t total = (int64_t)(s.groups + s.lag) * (s.nT + s.nG);
     const int64_t slots = (int64_t)p->sm_count * ctas_per_sm;
     kern<<<(unsigned)(total < slots ? total : slots), kThreads, 0, stream>>>(prm);
     HS_CUDA_OK(cudaGetLastError());
@@ -462,7 +469,7 @@ bool hs_interleaved_supported(const hs_plan *p)
     if (p->variant != HS_FREQBIN) return false;
     if (p->nbins > ((int64_t)1 << 18)) return false;
     const il_sched s = make_sched(p, p->batch);
-    return ((int64_t)s.groups + kLag) * (s.nT + s.nG) < ((int64_t)1 << 30);
+    return ((int64_t)s.groups + s.lag) * (s.nT + s.nG) < ((int64_t)1 << 30);
 }
 
 size_t hs_interleaved_workspace_bytes(const hs_plan *p, int64_t batch)

@@ -78,6 +78,10 @@ int hs_grouped_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, vo
 int hs_grouped_launches(const hs_plan *p, int64_t batch);
 size_t hs_grouped_workspace_bytes(const hs_plan *p, int64_t batch);
 bool hs_grouped_supported(const hs_plan *p);
+int hs_streamed_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
+int hs_streamed_launches(const hs_plan *p, int64_t batch);
+size_t hs_streamed_workspace_bytes(const hs_plan *p, int64_t batch);
+bool hs_streamed_supported(const hs_plan *p);
 
 // ---- device-side epilogue ---------------------------------------------------------------------------------------
 // c_H = fp32(1/sqrt(H)) for H = 1,2,4,8,16,32 (CONVENTIONS.md C7; "1/sqrt(H)").

@@ -15,7 +15,7 @@ from parity import argmax_from_levels, check_argmax, check_sums
 pytestmark = pytest.mark.gpu
 
 VARIANTS = ["standard", "max", "freqbin", "greedy"]
-ALGOS = ["direct", "tiled", "twophase", "gather", "grouped"]
+ALGOS = ["direct", "tiled", "twophase", "gather", "grouped", "streamed"]
 
 
 @pytest.fixture(scope="module")
@@ -30,8 +30,8 @@ def hs():
 
 def make_plan(hs, N, B, Hmax, variant, out_mode, algo):
     plan = hs.hs_plan_create(N, B, Hmax, variant, out_mode)
-    if algo in ("tiled", "twophase", "gather", "grouped"):
-        if algo in ("twophase", "grouped") and variant not in ("max", "freqbin"):
+    if algo in ("tiled", "twophase", "gather", "grouped", "streamed"):
+        if algo in ("twophase", "grouped", "streamed") and variant not in ("max", "freqbin"):
             pytest.skip("the two-phase kernels cover eqs. 2-3 only")
         if algo == "gather" and variant not in ("freqbin", "greedy"):
             pytest.skip("the plain gather kernel covers eqs. 3-4 only")
@@ -229,7 +229,7 @@ def test_error_paths_on_device(hs):
     assert e.value.code == hs.HS_ERR_INVALID_ARG
     assert plan.launches() >= 1 and plan.levels == 6
     with pytest.raises(hs.HsError):
-        plan.set_algo(7)
+        plan.set_algo(8)
     with pytest.raises(hs.HsError):
         g.set_algo("twophase")            # eq. 1 has no two-phase kernel
 
