@@ -32,15 +32,19 @@
 
 namespace {
 
-constexpr int G = 16;                                   // spectra per group = floats per row of xT
+#ifndef HS_IL_G
+#define HS_IL_G 16
+#endif
+constexpr int G = HS_IL_G;                                   // spectra per group = floats per row of xT
 constexpr int C = 4;                                    // consecutive bins per gather thread (times 4 spectra)
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kWarpBins = 8 * C;                        // 32 bins per warp
+constexpr int kLPR = G / 4;                              // lanes per row of xT (one float4 = 4 spectra each)
+constexpr int kWarpBins = (32 / kLPR) * C;              // bins per warp
 constexpr int kGTile = kWarps * kWarpBins;              // 256 bins per gather tile
 constexpr int kGSub = 2;                                // tiles per G item above the heavy region (bins >= N/8), 1 below
 constexpr int kLagDefault = 2;                          // the gather runs `lag` steps behind the copy
-constexpr int kTBins = 512;                             // bins per T item
+constexpr int kTBins = 512 * 16 / G;                    // bins per T item (32 KiB of input)
 constexpr int kTStride = kTBins + 4;                    // shared-memory row stride (floats) of the copy tile
 constexpr int kMaxRing = 4;
 
@@ -146,11 +150,11 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
     }
     __syncthreads();
     // thread t writes the float4 of spectra 4 (t % 4) .. +3 at bins k0 + t / 4 + 64 q
-    const int g4 = (threadIdx.x & 3) * 4;
+    const int g4 = (threadIdx.x & (kLPR - 1)) * 4;
     const int sw = g4 & 8;
 #pragma unroll
-    for (int q = 0; q < kTBins / (kThreads / 4); q++) {
-        const int kk = q * (kThreads / 4) + (threadIdx.x >> 2);
+    for (int q = 0; q < kTBins / (kThreads / kLPR); q++) {
+        const int kk = q * (kThreads / kLPR) + (threadIdx.x / kLPR);
         if (k0 + kk < N) {
             const float *t = tile + g4 * kTStride + (kk ^ sw);
             const float4 o = make_float4(t[0], t[kTStride], t[2 * kTStride], t[3 * kTStride]);
@@ -168,11 +172,11 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
 {
     const int N = p.N;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int q4 = lane & 3;                                           // spectra 4 q4 .. 4 q4 + 3 of the group
+    const int q4 = lane & (kLPR - 1);                                           // spectra 4 q4 .. 4 q4 + 3 of the group
     const int n_w = n_cta + warp * kWarpBins;                          // first bin of this warp
     const int n_end = min(N, p.n_split);                               // bins [n_end, N) belong to the T items
     if (n_w >= n_end) return;                                          // (warp-uniform)
-    const int n0 = n_w + (lane >> 2) * C;                              // first bin of this thread
+    const int n0 = n_w + (lane / kLPR) * C;                              // first bin of this thread
     const int n_hi1 = min(n_w + kWarpBins, n_end);                     // one past the warp's last bin
     const bool whole = n_w + kWarpBins <= n_end;                       // every lane's C bins exist
     const int64_t b0 = (int64_t)grp * G + 4 * q4;                      // first of this thread's spectra
