@@ -53,6 +53,9 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
+    ap.add_argument("--sweep", default="", choices=["", "scaling"],
+                    help="scaling: configs[4] throughput sweep over Hmax and spectrum length (one JSON line per point)")
+    ap.add_argument("--sweep-gib", type=float, default=16.0, help="fp32 input per sweep point (configs[4]: 16 GiB)")
     return ap.parse_args()
 
 
@@ -182,10 +185,57 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_scaling(args):
+    """--sweep scaling: BASELINE.json configs[4], scaling part.  Exp(1)-1 noise, nbins = 2^16 .. 2^24, batch sized to
+    --sweep-gib of fp32 input, Hmax = 2 .. 32, reduced output; per point and variant the median CUDA-event time of 5
+    launches after 3 warm-ups.  One JSON line per point (not the driver's contract line)."""
+    import torch
+
+    import workloads as W
+    from paper_1812_02647_b200 import binding as hs
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    peak, _ = measured_peak()
+    variants = args.variants.split(",")
+    words = int(args.sweep_gib * (1 << 30)) // 4
+    x_all = W.exp_noise_torch(1, words, 4, dev).view(-1)
+    vmax_all = torch.empty(words, dtype=torch.float32, device=dev)
+    amax_all = torch.empty(words, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    for lg in range(16, 25):
+        nbins = 1 << lg
+        batch = max(1, words // nbins)
+        x, vmax, amax = (t[:batch * nbins].view(batch, nbins) for t in (x_all, vmax_all, amax_all))
+        for Hmax in (2, 4, 8, 16, 32):
+            point = {"sweep": "scaling", "nbins": nbins, "batch": batch, "Hmax": Hmax, "out_mode": "reduced",
+                     "input_GiB": batch * nbins * 4 / 2**30, "per_variant": {}}
+            for v in variants:
+                p = hs.hs_plan_create(nbins, batch, Hmax, v, "reduced")
+                p.ensure_workspace(dev)
+                ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+                for _ in range(3):
+                    p.hs_execute(x, None, vmax, amax, stream)
+                for e0, e1 in ev:
+                    e0.record(stream)
+                    p.hs_execute(x, None, vmax, amax, stream)
+                    e1.record(stream)
+                torch.cuda.synchronize()
+                ms = statistics.median(e0.elapsed_time(e1) for e0, e1 in ev)
+                gbs = 9.0 * batch * nbins / (ms * 1e-3) / 1e9
+                point["per_variant"][v] = {"ms": ms, "bins_per_s": batch * nbins / (ms * 1e-3), "eff_GBps": gbs,
+                                           "frac_of_measured_peak": gbs / peak, "launches": p.launches(),
+                                           "workspace_MiB": round(p.workspace_bytes() / 2**20)}
+                p.hs_destroy()
+                del p
+            print(json.dumps(point), flush=True)
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep == "scaling":
+        return run_scaling(args)
 
     import numpy as np
     import torch

@@ -163,7 +163,9 @@ int hs_plan_set_algo(hs_plan *p, int algo)
     if ((algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GROUPED || algo == HS_ALGO_STREAMED) && p->variant != HS_MAX &&
         p->variant != HS_FREQBIN)
         HS_FAIL(HS_ERR_INVALID_ARG);
-    if (algo == HS_ALGO_GATHER && p->variant != HS_GREEDY && p->variant != HS_FREQBIN) HS_FAIL(HS_ERR_INVALID_ARG);
+    if (algo == HS_ALGO_GATHER && p->variant != HS_GREEDY && p->variant != HS_FREQBIN &&
+        !(p->variant == HS_MAX && p->Hmax <= 4))
+        HS_FAIL(HS_ERR_INVALID_ARG);
     const int before = p->algo_req;
     p->algo_req = algo;
     if ((algo == HS_ALGO_TILED || algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GATHER || algo == HS_ALGO_GROUPED ||

@@ -13,17 +13,58 @@
 namespace {
 
 constexpr int kThreads = 128;
-constexpr int kSpectraPerCta = 8;  // spectra run side by side per thread (tuned on B200: 2 -> 5.6 ms, 4 -> 4.9, 8 -> 4.7, 16 -> 5.4 for eq. 3)
+constexpr int kSpectraPerCta = 8;  // default Q; spectra run side by side per thread (tuned on B200: 2 -> 5.6 ms, 4 -> 4.9, 8 -> 4.7, 16 -> 5.4 for eq. 3)
 constexpr int kGridY = 65535; // blockIdx.y = spectrum: CTAs are dispatched x-fastest, i.e. spectrum-major, so the gathers of
                               // all harmonics of one spectrum (1 MiB) happen close in time and hit L2 (ncu: 4 B/bin of DRAM
                               // reads; striding spectra over a small gridDim.y instead thrashed L2 at 28-33 B/bin)
 
-template <int VARIANT, int L, int OUT>
-__global__ void __launch_bounds__(kThreads, 8)
+// eq. 2 term of harmonic I at bin n, every element in range: max x[I n .. I n + I - 1], widest aligned vector loads
+template <int I>
+__device__ __forceinline__ float max_window(const float *__restrict__ w)
+{
+    if constexpr (I % 4 == 0) {
+        float m = 0.f;
+#pragma unroll
+        for (int q = 0; q < I / 4; q++) {
+            const float4 u = __ldg(reinterpret_cast<const float4 *>(w) + q);
+            const float t = fmaxf(fmaxf(u.x, u.y), fmaxf(u.z, u.w));
+            m = q == 0 ? t : fmaxf(m, t);
+        }
+        return m;
+    } else if constexpr (I % 2 == 0) {
+        float m = 0.f;
+#pragma unroll
+        for (int q = 0; q < I / 2; q++) {
+            const float2 u = __ldg(reinterpret_cast<const float2 *>(w) + q);
+            const float t = fmaxf(u.x, u.y);
+            m = q == 0 ? t : fmaxf(m, t);
+        }
+        return m;
+    } else {
+        float m = __ldg(w);
+#pragma unroll
+        for (int q = 1; q < I; q++) m = fmaxf(m, __ldg(w + q));
+        return m;
+    }
+}
+__device__ __forceinline__ float max_window_rt(const float *__restrict__ w, int i)
+{
+    switch (i) {
+        case 2: return max_window<2>(w);
+        case 3: return max_window<3>(w);
+        case 4: return max_window<4>(w);
+        case 5: return max_window<5>(w);
+        case 6: return max_window<6>(w);
+        case 7: return max_window<7>(w);
+        default: return max_window<8>(w);
+    }
+}
+
+template <int VARIANT, int L, int OUT, int Q>
+__global__ void __launch_bounds__(kThreads, Q >= 8 ? 8 : 12)
 hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
                         uint8_t *__restrict__ amax, int N, int batch)
 {
-    constexpr int Q = kSpectraPerCta;
     const int n = blockIdx.x * kThreads + threadIdx.x;
     const int n_lo = n & ~31;                      // first bin of this warp
     if (n_lo >= N) return;
@@ -55,11 +96,19 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
                 if (OUT & HS_OUT_REDUCED) e[q].reduce(l, h);
             }
         };
-        auto step = [&](int base, bool safe) {      // harmonic with i * n == base
+        auto step = [&](int base, int i, bool safe) {   // harmonic i, i * n == base
 #pragma unroll
             for (int q = 0; q < Q; q++) {
                 if (VARIANT == HS_FREQBIN) {        // eq. 3: x~(i n)
                     S[q] += (safe || base < N) ? __ldg(xb[q] + base) : 0.0f;
+                } else if (VARIANT == HS_MAX) {     // eq. 2 (Hmax <= 8): maximum of the aligned block x~[i n .. i n + i - 1]
+                    if (safe) {
+                        S[q] += max_window_rt(xb[q] + base, i);
+                    } else {
+                        float m = base < N ? __ldg(xb[q] + base) : 0.0f;
+                        for (int t = 1; t < i; t++) m = fmaxf(m, base + t < N ? __ldg(xb[q] + base + t) : 0.0f);
+                        S[q] += m;
+                    }
                 } else {                            // eq. 4: max of the bin under the drift and its right neighbour
                     const int k = base + j[q];
                     const float lft = (safe || k < N) ? __ldg(xb[q] + k) : 0.0f;
@@ -80,11 +129,11 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
                 int base = (lo - 1) * nn;           // (i - 1) * n
                 for (; i <= hi && i * n_hi1 <= N; i++) {
                     base += nn;
-                    step(base, true);
+                    step(base, i, true);
                 }
                 for (; i <= hi && i * n_lo < N; i++) {
                     base += nn;
-                    step(base, false);
+                    step(base, i, false);
                 }
                 emit(l);
             } else if (OUT != HS_OUT_REDUCED) {
@@ -108,8 +157,8 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
     }
 }
 
-template <int VARIANT, int L, int OUT>
-int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+template <int VARIANT, int L, int OUT, int Q>
+int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     const int N = (int)p->nbins;
     const int tiles = (N + kThreads - 1) / kThreads;
@@ -117,14 +166,26 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
     for (int64_t b0 = 0; b0 < batch; b0 += max_spectra) {
         const int64_t nb = (batch - b0 < max_spectra) ? batch - b0 : max_spectra;
         const int64_t off = b0 * (int64_t)N;
-        const int64_t gy = (nb + kSpectraPerCta - 1) / kSpectraPerCta;
+        const int64_t gy = (nb + Q - 1) / Q;
         const dim3 grid((unsigned)tiles, (unsigned)(gy < kGridY ? gy : kGridY), 1);
-        hs_greedy_gather_kernel<VARIANT, L, OUT><<<grid, kThreads, 0, stream>>>(
+        hs_greedy_gather_kernel<VARIANT, L, OUT, Q><<<grid, kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
             buf.amax ? buf.amax + off : nullptr, N, (int)nb);
         HS_CUDA_OK(cudaGetLastError());
     }
     return HS_OK;
+}
+
+// Spectra side by side per thread: 8 while 8 spectra (and what is in flight around them) stay in L2; long spectra run
+// fewer at a time so that the gathers of all harmonics of a spectrum still hit L2 (2^22 bins = 16 MiB per spectrum).
+template <int VARIANT, int L, int OUT>
+int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+{
+    if (L >= 5) {                                                  // (with few harmonics the loads in flight matter more)
+        if (p->nbins > ((int64_t)1 << 22)) return launch_q<VARIANT, L, OUT, 1>(p, buf, batch, stream);
+        if (p->nbins > ((int64_t)1 << 20)) return launch_q<VARIANT, L, OUT, 2>(p, buf, batch, stream);
+    }
+    return launch_q<VARIANT, L, OUT, kSpectraPerCta>(p, buf, batch, stream);
 }
 
 template <int VARIANT, int L>
@@ -156,6 +217,14 @@ static int by_level(const hs_plan *p, const hs_buffers &buf, int64_t batch, cuda
 int hs_greedy_gather_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     if (p->variant == HS_FREQBIN) return by_level<HS_FREQBIN>(p, buf, batch, stream);
+    if (p->variant == HS_MAX) {                                    // Hmax <= 8 only (hs_tiled.cu)
+        switch (p->L) {
+            case 1: return by_out<HS_MAX, 1>(p, buf, batch, stream);
+            case 2: return by_out<HS_MAX, 2>(p, buf, batch, stream);
+            case 3: return by_out<HS_MAX, 3>(p, buf, batch, stream);
+            default: return by_out<HS_MAX, 4>(p, buf, batch, stream);
+        }
+    }
     return by_level<HS_GREEDY>(p, buf, batch, stream);
 }
 

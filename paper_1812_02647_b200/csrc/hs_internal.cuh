@@ -62,7 +62,8 @@ bool hs_tiled_supported(const hs_plan *p);
 // per-variant tuned kernels
 int hs_standard_tiled_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream);
 int hs_standard_tiled_launches(const hs_plan *p, int64_t batch);
-int hs_standard_rb_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream);
+int hs_standard_rb_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
+size_t hs_standard_rb_workspace_bytes(const hs_plan *p);
 bool hs_standard_rb_supported(const hs_plan *p);
 int hs_twophase_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
 int hs_twophase_launches(const hs_plan *p, int64_t batch);

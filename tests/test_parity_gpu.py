@@ -33,8 +33,8 @@ def make_plan(hs, N, B, Hmax, variant, out_mode, algo):
     if algo in ("tiled", "twophase", "gather", "grouped", "streamed"):
         if algo in ("twophase", "grouped", "streamed") and variant not in ("max", "freqbin"):
             pytest.skip("the two-phase kernels cover eqs. 2-3 only")
-        if algo == "gather" and variant not in ("freqbin", "greedy"):
-            pytest.skip("the plain gather kernel covers eqs. 3-4 only")
+        if algo == "gather" and variant not in ("freqbin", "greedy") and not (variant == "max" and Hmax <= 4):
+            pytest.skip("the plain gather kernel covers eqs. 3-4, and eq. 2 up to Hmax = 4")
         try:
             plan.set_algo(algo)
         except hs.HsError:
