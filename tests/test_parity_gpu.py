@@ -289,3 +289,17 @@ def test_host_buffer_entry_matches_device_entry(hs, variant, out_mode):
     assert torch.equal(h_max, vmax_d.cpu()) and torch.equal(h_amax, amax_d.cpu())
     if h_sums is not None:
         assert torch.equal(h_sums, sums_d.cpu())
+
+
+def test_sensitivity_sweep_small_instance(hs):
+    """configs[4] sensitivity harness on 24 realisations: on a Fourier bin freq-bin recovers what the standard sum does,
+    half a bin off it loses clearly more than Max HRMS does."""
+    from paper_1812_02647_b200 import sensitivity
+    res = sensitivity.run(realisations=24, snr=8.0, deltas=[0.0, 0.5], duties=[0.02])
+    on, off = res["points"]
+    assert on["delta"] == 0.0 and off["delta"] == 0.5
+    assert abs(on["snr"]["freqbin"] / on["snr"]["standard"] - 1.0) < 0.1
+    assert off["snr"]["freqbin"] < 0.75 * on["snr"]["freqbin"]
+    assert off["snr"]["max"] > 0.8 * on["snr"]["max"]
+    for p in (on, off):
+        assert p["snr"]["standard"] >= p["snr"]["max"] - 0.5
