@@ -128,6 +128,27 @@ size_t hs_plan_host_staging_bytes(const hs_plan *plan, int64_t slab_spectra);
 int hs_plan_set_host_staging(hs_plan *plan, void *d_staging, size_t bytes, int64_t slab_spectra);
 
 /*
+ * hs_execute_candidates — the path with the step that follows it in the pipeline fused in (the harmonic
+ * sum feeds SNR detection / candidate selection): instead of writing the reduced pair for every bin (5 bytes/bin), emit
+ * only the bins whose maximum over the levels exceeds `threshold`:
+ *     for every spectrum b and bin n with m(b, n) = max_l h_{2^l}(b, n) > threshold (strictly):
+ *         append { b, n, m(b, n), a(b, n) }          (m and a exactly as d_max / d_argmax of hs_execute, CONVENTIONS.md C8)
+ * The plan must have out_mode HS_OUT_REDUCED (else HS_ERR_INVALID_ARG); workspace rules as hs_execute.
+ *   d_cand     DEVICE, 16-byte aligned, room for `capacity` records; the ORDER of the records is unspecified
+ *   d_count    DEVICE, 8-byte aligned; zeroed by the call on `stream`, afterwards the number of bins above the threshold.
+ *              If it exceeds `capacity` only `capacity` records were kept (which ones is unspecified).
+ * Asynchronous on `stream` like hs_execute.  A low threshold makes the appends (one atomic each) the bottleneck.
+ */
+typedef struct hs_candidate {
+    int32_t spectrum; /* b */
+    int32_t bin;      /* n */
+    float value;      /* m(b, n) */
+    int32_t level;    /* a(b, n): level index l = log2 H of the best level, smallest on ties */
+} hs_candidate;
+int hs_execute_candidates(const hs_plan *plan, const float *d_x, float threshold, hs_candidate *d_cand,
+                          int64_t capacity, unsigned long long *d_count, void *stream);
+
+/*
  * hs_debug_greedy_paths — test-only: Greedy's drift j after each level, d_j[batch][L][nbins] uint8 (DEVICE),
  * because BASELINE.json north_star asks for bit-exact j paths and the production outputs do not expose j.
  * Valid for HS_GREEDY plans only (else HS_ERR_INVALID_ARG).  Not on the timed path.

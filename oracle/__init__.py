@@ -2,8 +2,10 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
 import this.  It never imports paper_1812_02647_b200 and shares nothing with it.
-All arithmetic lives in hs_oracle.c; this file only builds it (gcc -O2, no -ffast-math),
-marshals NumPy arrays and names the variants as the paper does.
+All arithmetic of eqs. 1-4 lives in hs_oracle.c; this file only builds it (gcc -O2, no -ffast-math),
+marshals NumPy arrays and names the variants as the paper does.  The one
+definition written here is candidates(): the threshold selection that follows the harmonic sum
+in the pipeline, stated on the reduced output the C code returns.
 """
 from __future__ import annotations
 
@@ -127,3 +129,18 @@ def partial_sum(x, n: int, H: int, variant):
     S = _load().hso_partial_sum(x.ctypes.data, x.shape[0], int(n), int(H), _variant(variant),
                                 ctypes.byref(j))
     return S, j.value
+
+
+def candidates(x, Hmax: int, variant, threshold: float) -> dict:
+    """The step after the harmonic sum ("SNR detection", "SNR recovered"): every (spectrum b,
+    bin n) whose maximum over the levels m(b, n) = max_l h_{2^l}(b, n) exceeds `threshold` strictly, with that maximum
+    and its level (smallest on ties, CONVENTIONS.md C8).  Plain definition: the reduced output of harmonic_sum, then a
+    comparison.  Returns spectrum[], bin[] (int64, sorted by (spectrum, bin)), value[] f64, level[] u8, and `margin[]`
+    = |m - threshold| for every bin of the batch as [B][N] f64 (so that a comparison can set aside the bins that sit
+    within rounding of the threshold)."""
+    ref = harmonic_sum(x, Hmax, variant, want_sums=False, want_reduced=True)
+    m = ref["max"]
+    b, n = np.nonzero(m > float(threshold))
+    return {"spectrum": b.astype(np.int64), "bin": n.astype(np.int64), "value": m[b, n], "level": ref["argmax"][b, n],
+            "margin": np.abs(m - float(threshold)), "gap": ref["gap"], "second": ref["second"], "max": m,
+            "argmax_all": ref["argmax"]}

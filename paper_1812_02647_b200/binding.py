@@ -43,6 +43,7 @@ _SIGS = {
     "hs_plan_host_staging_bytes": ([_p, _i64], _sz),
     "hs_plan_set_host_staging": ([_p, _p, _sz, _i64], _int),
     "hs_debug_greedy_paths": ([_p, _p, _p, _p], _int),
+    "hs_execute_candidates": ([_p, _p, ctypes.c_float, _p, _i64, _p, _p], _int),
 }
 for _name, (_args, _res) in _SIGS.items():
     _f = getattr(lib, _name)
@@ -141,6 +142,11 @@ class Plan:
     def hs_debug_greedy_paths(self, d_x, d_j, stream=None):
         _check(lib.hs_debug_greedy_paths(self.handle, _ptr(d_x), _ptr(d_j), _stream(stream)), "hs_debug_greedy_paths")
 
+    def hs_execute_candidates(self, d_x, threshold, d_cand, capacity, d_count, stream=None):
+        """d_cand: int32 CUDA tensor [capacity][4] (records spectrum, bin, value bits, level); d_count: int64 CUDA tensor [1]."""
+        _check(lib.hs_execute_candidates(self.handle, _ptr(d_x), ctypes.c_float(threshold), _ptr(d_cand), int(capacity),
+                                         _ptr(d_count), _stream(stream)), "hs_execute_candidates")
+
     def hs_destroy(self):
         if self.handle:
             lib.hs_destroy(self.handle)
@@ -167,3 +173,16 @@ class Plan:
         self.ensure_workspace(d_x.device)
         self.hs_execute(d_x, sums, vmax, amax, stream)
         return sums, vmax, amax
+
+    def run_candidates(self, d_x, threshold, capacity=1 << 20, stream=None):
+        """Allocate the candidate buffer, execute, return (count, records) with records = dict of torch tensors
+        (spectrum, bin, level: int32; value: float32), the first min(count, capacity) appended records, any order."""
+        import torch
+        cand = torch.empty((max(1, capacity), 4), dtype=torch.int32, device=d_x.device)
+        count = torch.zeros(1, dtype=torch.int64, device=d_x.device)
+        self.ensure_workspace(d_x.device)
+        self.hs_execute_candidates(d_x, threshold, cand, capacity, count, stream)
+        torch.cuda.synchronize()
+        n = int(count.item())
+        rec = cand[:min(n, capacity)]
+        return n, {"spectrum": rec[:, 0], "bin": rec[:, 1], "value": rec[:, 2].view(torch.float32), "level": rec[:, 3]}

@@ -220,6 +220,26 @@ int hs_execute(const hs_plan *p, const float *d_x, float *d_sums, float *d_max, 
     return launch_family(p, buf, p->batch, p->ws, static_cast<cudaStream_t>(stream));
 }
 
+int hs_execute_candidates(const hs_plan *p, const float *d_x, float threshold, hs_candidate *d_cand, int64_t capacity,
+                          unsigned long long *d_count, void *stream)
+{
+    if (!p || !d_x || !d_count || (!d_cand && capacity > 0)) HS_FAIL(HS_ERR_NULL_POINTER);
+    if (p->out_mode != HS_OUT_REDUCED || capacity < 0 || !(threshold == threshold)) HS_FAIL(HS_ERR_INVALID_ARG);
+    if (!aligned(d_x, 16) || !aligned(d_cand, 16) || !aligned(d_count, 8)) HS_FAIL(HS_ERR_MISALIGNED);
+    if (hs_plan_workspace_bytes(p) > 0 && (!p->ws || p->ws_bytes < hs_plan_workspace_bytes(p))) HS_FAIL(HS_ERR_WORKSPACE);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    HS_CUDA_OK(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s));
+    hs_buffers buf{d_x, nullptr, nullptr, nullptr, nullptr, {}};
+    // a kernel tests `cand` to choose between appending and storing: with no room at all it still has to count
+    static hs_candidate *const kNowhere = reinterpret_cast<hs_candidate *>(16);
+    buf.sink.cand = capacity > 0 ? d_cand : kNowhere;
+    buf.sink.count = d_count;
+    buf.sink.cap = capacity;
+    buf.sink.thr = threshold;
+    buf.sink.b0 = 0;
+    return launch_family(p, buf, p->batch, p->ws, s);
+}
+
 int hs_debug_greedy_paths(const hs_plan *p, const float *d_x, uint8_t *d_j, void *stream)
 {
     if (!p || !d_x || !d_j) HS_FAIL(HS_ERR_NULL_POINTER);

@@ -15,7 +15,7 @@ __device__ __forceinline__ float ldz(const float *__restrict__ x, int k, int N)
 template <int VARIANT, int L, int OUT, bool JDBG>
 __global__ void __launch_bounds__(kThreads)
 hs_direct_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
-                 uint8_t *__restrict__ amax, uint8_t *__restrict__ jdbg, int N, int tiles_per_spectrum)
+                 uint8_t *__restrict__ amax, uint8_t *__restrict__ jdbg, int N, int tiles_per_spectrum, hs_cand_sink sink)
 {
     const int64_t b = blockIdx.x / tiles_per_spectrum;
     const int n = (blockIdx.x % tiles_per_spectrum) * kThreads + threadIdx.x;
@@ -74,8 +74,12 @@ hs_direct_kernel(const float *__restrict__ x, float *__restrict__ sums, float *_
         }
     }
     if (OUT & HS_OUT_REDUCED) {
-        vmax[b * (int64_t)N + n] = e.m;
-        amax[b * (int64_t)N + n] = (uint8_t)e.a;
+        if (sink.cand) {
+            hs_push(sink, b, n, e.m, e.a);
+        } else {
+            vmax[b * (int64_t)N + n] = e.m;
+            amax[b * (int64_t)N + n] = (uint8_t)e.a;
+        }
     }
 }
 
@@ -88,9 +92,11 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
     for (int64_t b0 = 0; b0 < batch; b0 += max_spectra) {
         const int64_t nb = (batch - b0 < max_spectra) ? batch - b0 : max_spectra;
         const int64_t off = b0 * (int64_t)N;
+        hs_cand_sink sink = buf.sink;
+        sink.b0 += (int)b0;
         hs_direct_kernel<VARIANT, L, OUT, JDBG><<<(unsigned)(nb * tiles), kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
-            buf.amax ? buf.amax + off : nullptr, buf.jdbg ? buf.jdbg + off * L : nullptr, N, tiles);
+            buf.amax ? buf.amax + off : nullptr, buf.jdbg ? buf.jdbg + off * L : nullptr, N, tiles, sink);
         HS_CUDA_OK(cudaGetLastError());
     }
     return HS_OK;

@@ -63,7 +63,7 @@ __device__ __forceinline__ float max_window_rt(const float *__restrict__ w, int 
 template <int VARIANT, int L, int OUT, int Q>
 __global__ void __launch_bounds__(kThreads, Q >= 8 ? 8 : 12)
 hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
-                        uint8_t *__restrict__ amax, int N, int batch)
+                        uint8_t *__restrict__ amax, int N, int batch, hs_cand_sink sink)
 {
     const int n = blockIdx.x * kThreads + threadIdx.x;
     const int n_lo = n & ~31;                      // first bin of this warp
@@ -148,7 +148,9 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
         if (OUT & HS_OUT_REDUCED) {
 #pragma unroll
             for (int q = 0; q < Q; q++) {
-                if (live[q]) {
+                if (live[q] && sink.cand) {
+                    hs_push(sink, b0 + q, n, e[q].m, e[q].a);
+                } else if (live[q]) {
                     hsptx::st_cs(vmax + (int64_t)(b0 + q) * N + n, e[q].m);
                     hsptx::st_cs(amax + (int64_t)(b0 + q) * N + n, (uint8_t)e[q].a);
                 }
@@ -168,9 +170,11 @@ int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_
         const int64_t off = b0 * (int64_t)N;
         const int64_t gy = (nb + Q - 1) / Q;
         const dim3 grid((unsigned)tiles, (unsigned)(gy < kGridY ? gy : kGridY), 1);
+        hs_cand_sink sink = buf.sink;
+        sink.b0 += (int)b0;
         hs_greedy_gather_kernel<VARIANT, L, OUT, Q><<<grid, kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
-            buf.amax ? buf.amax + off : nullptr, N, (int)nb);
+            buf.amax ? buf.amax + off : nullptr, N, (int)nb, sink);
         HS_CUDA_OK(cudaGetLastError());
     }
     return HS_OK;

@@ -85,6 +85,7 @@ struct gr_params {
     int nchunks;     // phase-A chunks per spectrum
     int ntiles;      // phase-B warp tiles per spectrum: they cover the bins below n_split
     int n_split;     // multiple of kChunk, >= N/2: the outputs of bins n >= n_split are emitted by phase A
+    hs_cand_sink sink;
     int dbg;         // experiments only: 1 skip phase A, 2 skip phase B, 4 skip the barriers
 };
 
@@ -423,8 +424,18 @@ __device__ __forceinline__ void emit_upper(const gr_params &p, const gr_smem &sm
                                          x4.z < 0.f ? x4.z * c : x4.z, x4.w < 0.f ? x4.w * c : x4.w);
             const uint32_t a = (x4.x < 0.f ? (uint32_t)(L - 1) : 0u) | (x4.y < 0.f ? (uint32_t)(L - 1) << 8 : 0u) |
                                (x4.z < 0.f ? (uint32_t)(L - 1) << 16 : 0u) | (x4.w < 0.f ? (uint32_t)(L - 1) << 24 : 0u);
-            hsptx::st_cs(reinterpret_cast<float4 *>(p.vmax + row + n), m);
-            hsptx::st_cs(reinterpret_cast<uint32_t *>(p.amax + row + n), a);
+            if (p.sink.cand) {
+                if (fmaxf(fmaxf(m.x, m.y), fmaxf(m.z, m.w)) > p.sink.thr) {
+                    const int64_t b = row / N;
+                    hs_push(p.sink, b, n, m.x, (int)(a & 255u));
+                    hs_push(p.sink, b, n + 1, m.y, (int)((a >> 8) & 255u));
+                    hs_push(p.sink, b, n + 2, m.z, (int)((a >> 16) & 255u));
+                    hs_push(p.sink, b, n + 3, m.w, (int)(a >> 24));
+                }
+            } else {
+                hsptx::st_cs(reinterpret_cast<float4 *>(p.vmax + row + n), m);
+                hsptx::st_cs(reinterpret_cast<uint32_t *>(p.amax + row + n), a);
+            }
         }
     }
 }
@@ -513,7 +524,15 @@ __device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__r
     // With S unchanged over the skipped levels, h_l = S c_l is monotone in l: for S >= 0 no later level can
     // exceed the running maximum, for S < 0 the last level is the largest.  Testing level L-1 alone is enough.
     if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
-    if ((OUT & HS_OUT_REDUCED) && live) {
+    if ((OUT & HS_OUT_REDUCED) && live && p.sink.cand) {
+        if (fmaxf(fmaxf(e0.m, e1.m), fmaxf(e2.m, e3.m)) > p.sink.thr) {
+            const int64_t b = row / N;
+            hs_push(p.sink, b, n, e0.m, e0.a);
+            hs_push(p.sink, b, n + 1, e1.m, e1.a);
+            hs_push(p.sink, b, n + 2, e2.m, e2.a);
+            hs_push(p.sink, b, n + 3, e3.m, e3.a);
+        }
+    } else if ((OUT & HS_OUT_REDUCED) && live) {
         hsptx::st_cs(reinterpret_cast<float4 *>(p.vmax + row + n), make_float4(e0.m, e1.m, e2.m, e3.m));
         hsptx::st_cs(reinterpret_cast<uint32_t *>(p.amax + row + n),
                      (uint32_t)e0.a | ((uint32_t)e1.a << 8) | ((uint32_t)e2.a << 16) | ((uint32_t)e3.a << 24));
@@ -695,6 +714,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.sums = buf.sums;
     prm.vmax = buf.vmax;
     prm.amax = buf.amax;
+    prm.sink = buf.sink;
     prm.lay = s.lay;
     prm.N = (int)p->nbins;
     prm.B = (int)batch;
@@ -893,7 +913,9 @@ st_phaseB_kernel(const __grid_constant__ gr_params p, int b0)
     st_static_for(level, std::make_integer_sequence<int, L - 1>{});
     // With S unchanged over the skipped levels h_l = S c_l is monotone in l: testing the last level alone is enough.
     if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
-    if ((OUT & HS_OUT_REDUCED) && live) {
+    if ((OUT & HS_OUT_REDUCED) && live && p.sink.cand) {
+        hs_push(p.sink, b, n, e.m, e.a);
+    } else if ((OUT & HS_OUT_REDUCED) && live) {
         hsptx::st_cs(p.vmax + (int64_t)b * N + n, e.m);
         hsptx::st_cs(p.amax + (int64_t)b * N + n, (uint8_t)e.a);
     }
@@ -932,6 +954,7 @@ int st_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, 
     prm.sums = buf.sums;
     prm.vmax = buf.vmax;
     prm.amax = buf.amax;
+    prm.sink = buf.sink;
     prm.lay = s.lay;
     prm.N = (int)p->nbins;
     prm.B = (int)batch;

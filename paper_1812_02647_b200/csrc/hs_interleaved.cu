@@ -57,6 +57,7 @@ struct il_params {
     int *ctrl;          // [0] work counter, [1] error flag, [2..5] wait statistics, [16 + g] T items done, [16 + groups + g] G items done
     int64_t slot_words;
     int N, B, groups, R, lag;
+    hs_cand_sink sink;
     int nT, nG;         // items per group
     int nHeavy;         // the first nHeavy G items are single tiles (bins below ~N/8: 8 to 32 harmonics per bin)
     int n_split;        // G items cover bins [0, n_split); T items emit the outputs of [n_split, N)
@@ -140,7 +141,14 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
                         e3.reduce(l, h.w);
                     }
                 }
-                if (OUT & HS_OUT_REDUCED) {
+                if ((OUT & HS_OUT_REDUCED) && p.sink.cand) {
+                    if (fmaxf(fmaxf(e0.m, e1.m), fmaxf(e2.m, e3.m)) > p.sink.thr) {
+                        hs_push(p.sink, b0 + g, k, e0.m, e0.a);
+                        hs_push(p.sink, b0 + g, k + 1, e1.m, e1.a);
+                        hs_push(p.sink, b0 + g, k + 2, e2.m, e2.a);
+                        hs_push(p.sink, b0 + g, k + 3, e3.m, e3.a);
+                    }
+                } else if (OUT & HS_OUT_REDUCED) {
                     hsptx::st_cs(reinterpret_cast<float4 *>(p.vmax + row + k), make_float4(e0.m, e1.m, e2.m, e3.m));
                     hsptx::st_cs(reinterpret_cast<uint32_t *>(p.amax + row + k),
                                  (uint32_t)e0.a | ((uint32_t)e1.a << 8) | ((uint32_t)e2.a << 16) | ((uint32_t)e3.a << 24));
@@ -288,7 +296,11 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
     if (OUT & HS_OUT_REDUCED) {
 #pragma unroll
         for (int q = 0; q < 4; q++) {
-            if (b0 + q < p.B) {
+            if (b0 + q < p.B && p.sink.cand) {
+#pragma unroll
+                for (int k = 0; k < C; k++)
+                    if (n0 + k < n_end) hs_push(p.sink, b0 + q, n0 + k, e[k][q].m, e[k][q].a);
+            } else if (b0 + q < p.B) {
                 float *pm = p.vmax + (b0 + q) * N + n0;
                 uint8_t *pa = p.amax + (b0 + q) * N + n0;
                 if (whole) {
@@ -417,6 +429,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.sums = buf.sums;
     prm.vmax = buf.vmax;
     prm.amax = buf.amax;
+    prm.sink = buf.sink;
     prm.slot_words = s.slot_words;
     prm.N = (int)p->nbins;
     prm.B = (int)batch;

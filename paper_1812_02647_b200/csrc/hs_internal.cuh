@@ -47,12 +47,22 @@ void hs_set_error(int code);
 
 // ---- launch entry points of the kernel families -------------------------------------------------------------------
 // Each enqueues on `stream` for spectra [0, batch) of the given buffers and returns an hs_status.
+// Candidate sink of hs_execute_candidates: when `cand` is set a kernel appends the bins whose reduced maximum exceeds
+// `thr` instead of storing vmax / amax (which are then nullptr).  `b0` = batch index of the first spectrum of the launch.
+struct hs_cand_sink {
+    hs_candidate *cand;
+    unsigned long long *count;
+    long long cap;
+    float thr;
+    int b0;
+};
 struct hs_buffers {
     const float *x;
     float *sums;
     float *vmax;
     uint8_t *amax;
     uint8_t *jdbg;  // Greedy debug paths or nullptr
+    hs_cand_sink sink;
 };
 int hs_launch_direct(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
 int hs_launch_tiled(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
@@ -94,6 +104,18 @@ __device__ __forceinline__ constexpr float hs_norm(int l)
          : l == 3 ? 0.35355339059327376220f
          : l == 4 ? 0.25f
                   : 0.17677669529663688110f;
+}
+
+// hs_execute_candidates: append (b, n, m, a) if m > thr.  Bins above a sensible threshold are rare, so one atomic each.
+__device__ __forceinline__ void hs_push(const hs_cand_sink &s, int64_t b, int n, float m, int a)
+{
+    if (m > s.thr) {
+        const unsigned long long pos = atomicAdd(s.count, 1ULL);
+        if (pos < (unsigned long long)s.cap) {
+            int4 rec = make_int4((int)(b + s.b0), n, __float_as_int(m), a);
+            *reinterpret_cast<int4 *>(s.cand + pos) = rec;
+        }
+    }
 }
 
 // Running reduced output of one bin: m = max_l h_l, a = smallest l attaining it (C8).

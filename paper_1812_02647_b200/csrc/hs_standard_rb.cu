@@ -55,6 +55,7 @@ struct rb_params {
     float *vmax;
     uint8_t *amax;
     int *counter;    // tile queue (zeroed before the launch)
+    hs_cand_sink sink;
     int N;
     int tiles_per_spectrum;
     int tiles;       // total (< 2^31: checked on the host)
@@ -194,6 +195,7 @@ rb_kernel(const __grid_constant__ rb_params p)
     issue(std::integral_constant<int, 0>{}, cb, ct, 0, cur < p.tiles);
     issue(std::integral_constant<int, 1>{}, cb, ct, 1, cur < p.tiles);
     issue(std::integral_constant<int, 2>{}, cb, ct, 2, cur < p.tiles);
+    if constexpr (kSlots > 3) issue(std::integral_constant<int, 3>{}, cb, ct, 3, cur < p.tiles);
 
     uint32_t phase = 0u;                                                  // bit s: parity of the next wait on full[s]
     float S[32], m[32];
@@ -236,6 +238,16 @@ rb_kernel(const __grid_constant__ rb_params p)
 
         // ---- outputs of the tile: thread holds bins nw0 + 32 lane + [0, 32)
         const int64_t base = b * N + n0 + warp * 1024;
+        if (p.sink.cand) {                                               // hs_execute_candidates: no stores, rare appends
+            float mm = m[0];
+#pragma unroll
+            for (int r = 1; r < 32; r++) mm = fmaxf(mm, m[r]);
+            if (mm > p.sink.thr) {
+#pragma unroll
+                for (int r = 0; r < 32; r++) hs_push(p.sink, b, n0 + warp * 1024 + 32 * lane + r, m[r], a[r]);
+            }
+            continue;
+        }
 #pragma unroll
         for (int h = 0; h < 2; h++) {
 #pragma unroll
@@ -285,6 +297,7 @@ int hs_standard_rb_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch
     prm.tiles_per_spectrum = (int)(p->nbins / kT);
     prm.tiles = (int)(batch * prm.tiles_per_spectrum);
     prm.counter = static_cast<int *>(ws);
+    prm.sink = buf.sink;
     const size_t smem = (size_t)(kSlots * kSlot + (kNT / 32) * 32 * kOutRow) * sizeof(float);
     static bool configured = false;
     if (!configured) {

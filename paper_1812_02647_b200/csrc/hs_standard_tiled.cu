@@ -17,7 +17,7 @@ constexpr int ilog2(int v) { return v <= 1 ? 0 : 1 + ilog2(v >> 1); }
 template <int HMAX, int OUT, int WARPS, int STEPS>
 __global__ void __launch_bounds__(WARPS * 32)
 hs_std_tiled_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
-                    uint8_t *__restrict__ amax, int N, int tiles)
+                    uint8_t *__restrict__ amax, int N, int tiles, hs_cand_sink sink)
 {
     constexpr int LG = ilog2(HMAX), L = LG + 1, T = WARPS * STEPS * 32;
     extern __shared__ __align__(128) float win[];
@@ -82,8 +82,12 @@ hs_std_tiled_kernel(const float *__restrict__ x, float *__restrict__ sums, float
                 e.level(l, S, plane0, N);
             }
             if (OUT & HS_OUT_REDUCED) {
-                hsptx::st_cs(vmax + b * (int64_t)N + n, e.m);
-                hsptx::st_cs(amax + b * (int64_t)N + n, (uint8_t)e.a);
+                if (sink.cand) {
+                    hs_push(sink, b, n, e.m, e.a);
+                } else {
+                    hsptx::st_cs(vmax + b * (int64_t)N + n, e.m);
+                    hsptx::st_cs(amax + b * (int64_t)N + n, (uint8_t)e.a);
+                }
             }
         }
     }
@@ -106,9 +110,11 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
     for (int64_t b0 = 0; b0 < batch; b0 += max_spectra) {
         const int64_t nb = (batch - b0 < max_spectra) ? batch - b0 : max_spectra;
         const int64_t off = b0 * (int64_t)N;
+        hs_cand_sink sink = buf.sink;
+        sink.b0 += (int)b0;
         kern<<<(unsigned)(nb * tiles), WARPS * 32, smem, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * p->L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
-            buf.amax ? buf.amax + off : nullptr, N, tiles);
+            buf.amax ? buf.amax + off : nullptr, N, tiles, sink);
         HS_CUDA_OK(cudaGetLastError());
     }
     return HS_OK;

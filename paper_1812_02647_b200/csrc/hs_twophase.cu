@@ -61,6 +61,7 @@ struct tp_params {
     float *sums;
     float *vmax;
     uint8_t *amax;
+    hs_cand_sink sink;
     int *ctrl;       // [0] work counter, [1] error flag, [2..5] wait statistics, [16 + b] phase-1 chunks done, [16 + B + b] phase-2 tiles done
     tp_layout lay;
     int N;
@@ -282,7 +283,15 @@ __device__ __forceinline__ void phase2_round(const tp_params &p, const float *__
     // With S unchanged over the skipped levels, h_l = S c_l is monotone in l: for S >= 0 no later level can
     // exceed the running maximum, for S < 0 the last level is the largest.  Testing level L-1 alone is enough.
     if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
-    if (OUT & HS_OUT_REDUCED) {
+    if ((OUT & HS_OUT_REDUCED) && p.sink.cand) {
+        if (fmaxf(fmaxf(e0.m, e1.m), fmaxf(e2.m, e3.m)) > p.sink.thr) {
+            const int64_t b = row / p.N;
+            hs_push(p.sink, b, n, e0.m, e0.a);
+            hs_push(p.sink, b, n + 1, e1.m, e1.a);
+            hs_push(p.sink, b, n + 2, e2.m, e2.a);
+            hs_push(p.sink, b, n + 3, e3.m, e3.a);
+        }
+    } else if (OUT & HS_OUT_REDUCED) {
         hsptx::st_cs(reinterpret_cast<float4 *>(p.vmax + row + n), make_float4(e0.m, e1.m, e2.m, e3.m));
         hsptx::st_cs(reinterpret_cast<uint32_t *>(p.amax + row + n),
                      (uint32_t)e0.a | ((uint32_t)e1.a << 8) | ((uint32_t)e2.a << 16) | ((uint32_t)e3.a << 24));
@@ -527,6 +536,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.sums = buf.sums;
     prm.vmax = buf.vmax;
     prm.amax = buf.amax;
+    prm.sink = buf.sink;
     prm.lay = s.lay;
     prm.N = (int)p->nbins;
     prm.B = (int)batch;

@@ -49,3 +49,28 @@ def argmax_from_levels(h):
     second = masked.argmax(axis=-1)
     gap = vmax - np.take_along_axis(masked, second[..., None], -1)[..., 0]
     return best, second, gap, vmax
+
+
+def check_candidates(count, got, ref, shape, what=""):
+    """Candidate lists (hs_execute_candidates vs oracle.candidates): the order is unspecified, so both are compared as
+    sets keyed by (spectrum, bin).  Every oracle candidate must be present and every record must be an oracle candidate,
+    except bins whose oracle maximum lies within the tolerance of the threshold (either side may have them); values
+    within the tolerance, levels by the rule of check_argmax.  `got` = dict of NumPy arrays (spectrum, bin, value, level)
+    holding ALL `count` records.  Returns the number of threshold-borderline bins that were set aside."""
+    B, N = shape
+    gs, gb = np.asarray(got["spectrum"]).astype(np.int64), np.asarray(got["bin"]).astype(np.int64)
+    assert count == gs.shape[0], f"{what}: count {count} != {gs.shape[0]} records"
+    assert ((gs >= 0) & (gs < B) & (gb >= 0) & (gb < N)).all(), f"{what}: record outside the batch"
+    gkey = gs * N + gb
+    assert np.unique(gkey).shape[0] == gkey.shape[0], f"{what}: a bin was appended twice"
+    rkey = np.asarray(ref["spectrum"]).astype(np.int64) * N + np.asarray(ref["bin"]).astype(np.int64)
+    border = (ref["margin"] <= TOL * (1.0 + np.abs(ref["max"]))).reshape(-1)
+    missing = np.setdiff1d(rkey, gkey)
+    extra = np.setdiff1d(gkey, rkey)
+    assert border[missing].all(), f"{what}: {int((~border[missing]).sum())} oracle candidates missing, e.g. {missing[:3]}"
+    assert border[extra].all(), f"{what}: {int((~border[extra]).sum())} records are no oracle candidates, e.g. {extra[:3]}"
+    m = ref["max"].reshape(-1)[gkey]
+    check_sums(np.asarray(got["value"]), m, what + " value")
+    check_argmax(np.asarray(got["level"]), (ref["argmax_all"]).reshape(-1)[gkey], ref["second"].reshape(-1)[gkey],
+                 ref["gap"].reshape(-1)[gkey], m, what + " level")
+    return int(missing.shape[0] + extra.shape[0])

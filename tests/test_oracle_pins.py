@@ -356,3 +356,28 @@ def test_points_entry_matches_whole_batch(oracle):
         np.testing.assert_array_equal(j, o["jpath"][b, :, n])
     with pytest.raises(ValueError):
         oracle.points(x, 16, "max", [4], [0])
+
+
+def test_candidates_definition_on_a_zero_background_comb():
+    """oracle.candidates (threshold detection after the harmonic sum): on a zero background with spikes
+    a_k at bins k m the freq-bin maximum over levels at bin m is max_H sum_{k<=H} a_k / sqrt(H); every bin above the
+    threshold is listed exactly once, sorted, with the level of the maximum; nothing else is."""
+    import oracle
+    N, m = 4096, 37
+    x = np.zeros((2, N), np.float32)
+    a = np.array([9.0, 7.0, 5.0, 3.0, 1.0, 1.0, 1.0, 1.0], np.float64)
+    for k in range(1, 9):
+        x[1, k * m] = a[k - 1]
+    h = [a[:H].sum() / np.sqrt(H) for H in (1, 2, 4, 8)]            # 9, 11.31, 12, 9.9 -> best level 2 (H = 4)
+    res = oracle.candidates(x, 8, "freqbin", 11.5)
+    assert res["spectrum"].tolist() == [1] and res["bin"].tolist() == [m]
+    assert abs(res["value"][0] - max(h)) < 1e-12 and res["level"][0] == int(np.argmax(h)) == 2
+    res = oracle.candidates(x, 8, "freqbin", 8.9)                    # the spike of 9 at bin m itself and at ... only m: 2m holds 7
+    assert res["bin"].tolist() == [m]
+    res = oracle.candidates(x, 8, "freqbin", 6.9)                    # bins m (12) and 2m (x = 7, harmonics 4m: 3, 6m: 1, 8m: 1)
+    assert res["spectrum"].tolist() == [1, 1] and res["bin"].tolist() == [m, 2 * m]
+    assert oracle.candidates(x, 8, "freqbin", 12.0)["bin"].size == 0  # strictly greater
+    full = oracle.harmonic_sum(x, 8, "freqbin")
+    ref = np.argwhere(full["sums"].max(axis=1) > 2.9)
+    res = oracle.candidates(x, 8, "freqbin", 2.9)
+    assert np.array_equal(np.stack([res["spectrum"], res["bin"]], 1), ref)

@@ -10,7 +10,7 @@ import pytest
 import torch
 
 import workloads as W
-from parity import argmax_from_levels, check_argmax, check_sums
+from parity import check_candidates, argmax_from_levels, check_argmax, check_sums
 
 pytestmark = pytest.mark.gpu
 
@@ -303,3 +303,44 @@ def test_sensitivity_sweep_small_instance(hs):
     assert off["snr"]["max"] > 0.8 * on["snr"]["max"]
     for p in (on, off):
         assert p["snr"]["standard"] >= p["snr"]["max"] - 0.5
+
+
+# ---------------------------------------------------------------------------------------------------- candidates (fused back end)
+def _records(rec):
+    return {k: v.cpu().numpy() for k, v in rec.items()}
+
+
+@pytest.mark.parametrize("algo", ["direct", "tiled", "twophase", "gather", "grouped", "streamed"])
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_candidates_match_the_oracle(hs, oracle, variant, algo):
+    """hs_execute_candidates against oracle.candidates on noise + combs: several tiles, ragged tail, both halves of the
+    spectrum (bins >= N/2 are emitted by other code than the bins below), thresholds from 'a few' to 'thousands'."""
+    for N, B, Hmax in ((20000, 3, 32), (1 << 15, 5, 32), (4100, 2, 8)):
+        x, _ = W.comb_batch_numpy(2, list(range(B)), N, 1.0, 50.0, 500.0, 0.10)
+        d_x = torch.from_numpy(x).cuda()
+        plan = make_plan(hs, N, B, Hmax, variant, "reduced", algo)
+        for thr in (2.5, 6.0, 40.0):
+            ref = oracle.candidates(x, Hmax, variant, thr)
+            count, rec = plan.run_candidates(d_x, thr, capacity=B * N)
+            check_candidates(count, _records(rec), ref, (B, N), f"{variant}/{algo}/N={N}/thr={thr}")
+        plan.hs_destroy()
+
+
+def test_candidates_capacity_count_and_errors(hs, oracle):
+    N, B = 1 << 14, 4
+    x, _ = W.comb_batch_numpy(2, list(range(B)), N, 1.0, 50.0, 500.0, 0.10)
+    d_x = torch.from_numpy(x).cuda()
+    plan = hs.hs_plan_create(N, B, 32, "freqbin", "reduced")
+    ref = oracle.candidates(x, 32, "freqbin", 3.0)
+    total = ref["spectrum"].shape[0]
+    assert total > 100
+    count, rec = plan.run_candidates(d_x, 3.0, capacity=64)          # more candidates than room: count is the total
+    assert abs(count - total) <= 2 and rec["bin"].shape[0] == 64
+    count0, _ = plan.run_candidates(d_x, 3.0, capacity=0)
+    assert abs(count0 - total) <= 2
+    count_none, rec_none = plan.run_candidates(d_x, 1e30, capacity=16)
+    assert count_none == 0 and rec_none["bin"].shape[0] == 0
+    full = hs.hs_plan_create(N, B, 32, "freqbin", "full")
+    with pytest.raises(hs.HsError) as e:
+        full.run_candidates(d_x, 3.0)
+    assert e.value.code == hs.HS_ERR_INVALID_ARG
