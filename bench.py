@@ -53,6 +53,8 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
+    ap.add_argument("--candidates-threshold", type=float, default=25.0,
+                    help="also time hs_execute_candidates at this threshold (0: skip); reported under \"candidates\"")
     ap.add_argument("--sweep", default="", choices=["", "scaling"],
                     help="scaling: configs[4] throughput sweep over Hmax and spectrum length (one JSON line per point)")
     ap.add_argument("--sweep-gib", type=float, default=16.0, help="fp32 input per sweep point (configs[4]: 16 GiB)")
@@ -342,6 +344,28 @@ def main():
         # other ranks still take part in the e2e collectives below
         pass
 
+    # ---- fused back end: hs_execute_candidates, 4 B/bin of HBM traffic instead of 9 -------------------
+    cand_line = None
+    if out_mode == "reduced" and args.candidates_threshold > 0:
+        cap = 1 << 22
+        d_cand = torch.empty((cap, 4), dtype=torch.int32, device=dev)
+        d_count = torch.zeros(1, dtype=torch.int64, device=dev)
+        cand_line = {"threshold": args.candidates_threshold, "algorithmic_bytes_per_bin": 4, "per_variant": {}}
+        for v in variants:
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(max(3, args.steps))]
+            for _ in range(3):
+                plans[v].hs_execute_candidates(x, args.candidates_threshold, d_cand, cap, d_count, stream)
+            for e0, e1 in ev:
+                e0.record(stream)
+                plans[v].hs_execute_candidates(x, args.candidates_threshold, d_cand, cap, d_count, stream)
+                e1.record(stream)
+            torch.cuda.synchronize()
+            ms = statistics.mean(e0.elapsed_time(e1) for e0, e1 in ev)
+            cand_line["per_variant"][v] = {"ms": ms, "bins_per_s": batch * nbins / (ms * 1e-3), "found": int(d_count.item()),
+                                           "eff_GBps": 4.0 * batch * nbins / (ms * 1e-3) / 1e9,
+                                           "frac_of_measured_peak": 4.0 * batch * nbins / (ms * 1e-3) / 1e9 / peak}
+        del d_cand
+
     # ---- e2e: the same step through hs_execute_host with pinned host buffers -------------------------------------------
     e2e = None
     if not args.no_e2e:
@@ -405,7 +429,7 @@ def main():
                            "input_checksum_spectrum0": W.checksum(x[:1].cpu().numpy())},
                 "eff_GBps": value * bpb / 1e9 / world, "frac_of_measured_peak": value * bpb / 1e9 / world / peak,
                 "frac_of_nominal_8TBps": value * bpb / 1e9 / world / 8000.0,
-                "per_variant": per_variant, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+                "per_variant": per_variant, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "candidates": cand_line,
                 "gpu_launches": sum(plans[v].launches() for v in variants) * args.steps, "clocks": clocks,
                 "paper_context": "PAPER.md:66-71 Table 1 GPU/CPU speed-ups 250x/704x/110x/177x (std/greedy/freq-bin/max), "
                                  "hardware not stated"}

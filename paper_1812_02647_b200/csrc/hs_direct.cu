@@ -74,7 +74,7 @@ hs_direct_kernel(const float *__restrict__ x, float *__restrict__ sums, float *_
         }
     }
     if (OUT & HS_OUT_REDUCED) {
-        if (sink.cand) {
+        if (OUT & HS_OUT_CAND) {
             hs_push(sink, b, n, e.m, e.a);
         } else {
             vmax[b * (int64_t)N + n] = e.m;
@@ -110,7 +110,9 @@ int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
     }
     switch (p->out_mode) {
         case HS_OUT_FULL: return launch<VARIANT, L, HS_OUT_FULL, false>(p, buf, batch, stream);
-        case HS_OUT_REDUCED: return launch<VARIANT, L, HS_OUT_REDUCED, false>(p, buf, batch, stream);
+        case HS_OUT_REDUCED:
+            if (buf.sink.cand) return launch<VARIANT, L, HS_OUT_REDUCED | HS_OUT_CAND, false>(p, buf, batch, stream);
+            return launch<VARIANT, L, HS_OUT_REDUCED, false>(p, buf, batch, stream);
         default: return launch<VARIANT, L, HS_OUT_BOTH, false>(p, buf, batch, stream);
     }
 }

@@ -136,7 +136,7 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
                     step(base, i, false);
                 }
                 emit(l);
-            } else if (OUT != HS_OUT_REDUCED) {
+            } else if ((OUT & 3) != HS_OUT_REDUCED) {
                 emit(l);
             } else {
                 tail = true;
@@ -144,11 +144,11 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
         }
         // Levels whose harmonics are all out of range leave S unchanged, and h_l = S c_l is monotone in l: for S >= 0
         // no later level exceeds the running maximum, for S < 0 the last level is the largest.  Test level L-1 only.
-        if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
+        if ((OUT & 3) == HS_OUT_REDUCED && tail) emit(L - 1);
         if (OUT & HS_OUT_REDUCED) {
 #pragma unroll
             for (int q = 0; q < Q; q++) {
-                if (live[q] && sink.cand) {
+                if (live[q] && (OUT & HS_OUT_CAND)) {
                     hs_push(sink, b0 + q, n, e[q].m, e[q].a);
                 } else if (live[q]) {
                     hsptx::st_cs(vmax + (int64_t)(b0 + q) * N + n, e[q].m);
@@ -197,7 +197,9 @@ int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
 {
     switch (p->out_mode) {
         case HS_OUT_FULL: return launch<VARIANT, L, HS_OUT_FULL>(p, buf, batch, stream);
-        case HS_OUT_REDUCED: return launch<VARIANT, L, HS_OUT_REDUCED>(p, buf, batch, stream);
+        case HS_OUT_REDUCED:
+            if (buf.sink.cand) return launch<VARIANT, L, HS_OUT_REDUCED | HS_OUT_CAND>(p, buf, batch, stream);
+            return launch<VARIANT, L, HS_OUT_REDUCED>(p, buf, batch, stream);
         default: return launch<VARIANT, L, HS_OUT_BOTH>(p, buf, batch, stream);
     }
 }

@@ -424,7 +424,7 @@ __device__ __forceinline__ void emit_upper(const gr_params &p, const gr_smem &sm
                                          x4.z < 0.f ? x4.z * c : x4.z, x4.w < 0.f ? x4.w * c : x4.w);
             const uint32_t a = (x4.x < 0.f ? (uint32_t)(L - 1) : 0u) | (x4.y < 0.f ? (uint32_t)(L - 1) << 8 : 0u) |
                                (x4.z < 0.f ? (uint32_t)(L - 1) << 16 : 0u) | (x4.w < 0.f ? (uint32_t)(L - 1) << 24 : 0u);
-            if (p.sink.cand) {
+            if (OUT & HS_OUT_CAND) {
                 if (fmaxf(fmaxf(m.x, m.y), fmaxf(m.z, m.w)) > p.sink.thr) {
                     const int64_t b = row / N;
                     hs_push(p.sink, b, n, m.x, (int)(a & 255u));
@@ -515,7 +515,7 @@ __device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__r
                 }
             }
             emit(l);
-        } else if (OUT != HS_OUT_REDUCED) {
+        } else if ((OUT & 3) != HS_OUT_REDUCED) {
             emit(l);
         } else {
             tail = true;
@@ -523,8 +523,8 @@ __device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__r
     }
     // With S unchanged over the skipped levels, h_l = S c_l is monotone in l: for S >= 0 no later level can
     // exceed the running maximum, for S < 0 the last level is the largest.  Testing level L-1 alone is enough.
-    if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
-    if ((OUT & HS_OUT_REDUCED) && live && p.sink.cand) {
+    if ((OUT & 3) == HS_OUT_REDUCED && tail) emit(L - 1);
+    if ((OUT & HS_OUT_REDUCED) && live && (OUT & HS_OUT_CAND)) {
         if (fmaxf(fmaxf(e0.m, e1.m), fmaxf(e2.m, e3.m)) > p.sink.thr) {
             const int64_t b = row / N;
             hs_push(p.sink, b, n, e0.m, e0.a);
@@ -747,7 +747,9 @@ int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
 {
     switch (p->out_mode) {
         case HS_OUT_FULL: return launch<VARIANT, HMAX, HS_OUT_FULL>(p, buf, batch, ws, stream);
-        case HS_OUT_REDUCED: return launch<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
+        case HS_OUT_REDUCED:
+            if (buf.sink.cand) return launch<VARIANT, HMAX, HS_OUT_REDUCED | HS_OUT_CAND>(p, buf, batch, ws, stream);
+            return launch<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
         default: return launch<VARIANT, HMAX, HS_OUT_BOTH>(p, buf, batch, ws, stream);
     }
 }
@@ -904,7 +906,7 @@ st_phaseB_kernel(const __grid_constant__ gr_params p, int b0)
             };
             st_static_for(harmonic, std::make_integer_sequence<int, hi - lo + 1>{});
             emit(l);
-        } else if (OUT != HS_OUT_REDUCED) {
+        } else if ((OUT & 3) != HS_OUT_REDUCED) {
             emit(l);
         } else {
             tail = true;
@@ -912,8 +914,8 @@ st_phaseB_kernel(const __grid_constant__ gr_params p, int b0)
     };
     st_static_for(level, std::make_integer_sequence<int, L - 1>{});
     // With S unchanged over the skipped levels h_l = S c_l is monotone in l: testing the last level alone is enough.
-    if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
-    if ((OUT & HS_OUT_REDUCED) && live && p.sink.cand) {
+    if ((OUT & 3) == HS_OUT_REDUCED && tail) emit(L - 1);
+    if ((OUT & HS_OUT_REDUCED) && live && (OUT & HS_OUT_CAND)) {
         hs_push(p.sink, b, n, e.m, e.a);
     } else if ((OUT & HS_OUT_REDUCED) && live) {
         hsptx::st_cs(p.vmax + (int64_t)b * N + n, e.m);
@@ -985,7 +987,9 @@ int st_by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, 
 {
     switch (p->out_mode) {
         case HS_OUT_FULL: return st_launch<VARIANT, HMAX, HS_OUT_FULL>(p, buf, batch, ws, stream);
-        case HS_OUT_REDUCED: return st_launch<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
+        case HS_OUT_REDUCED:
+            if (buf.sink.cand) return st_launch<VARIANT, HMAX, HS_OUT_REDUCED | HS_OUT_CAND>(p, buf, batch, ws, stream);
+            return st_launch<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
         default: return st_launch<VARIANT, HMAX, HS_OUT_BOTH>(p, buf, batch, ws, stream);
     }
 }

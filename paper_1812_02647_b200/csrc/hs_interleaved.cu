@@ -130,7 +130,7 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
 #pragma unroll
                 for (int l = 0; l < L; l++) {
                     // h_l = x c_l is monotone in l: in reduced-only mode the first and the last level decide
-                    if (OUT == HS_OUT_REDUCED && l != 0 && l != L - 1) continue;
+                    if ((OUT & 3) == HS_OUT_REDUCED && l != 0 && l != L - 1) continue;
                     const float4 h = make_float4(v[s][q].x * hs_norm(l), v[s][q].y * hs_norm(l), v[s][q].z * hs_norm(l),
                                                  v[s][q].w * hs_norm(l));
                     if (OUT & HS_OUT_FULL) hsptx::st_cs(reinterpret_cast<float4 *>(p.sums + (row * L + (int64_t)l * N + k)), h);
@@ -141,7 +141,7 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
                         e3.reduce(l, h.w);
                     }
                 }
-                if ((OUT & HS_OUT_REDUCED) && p.sink.cand) {
+                if ((OUT & HS_OUT_REDUCED) && (OUT & HS_OUT_CAND)) {
                     if (fmaxf(fmaxf(e0.m, e1.m), fmaxf(e2.m, e3.m)) > p.sink.thr) {
                         hs_push(p.sink, b0 + g, k, e0.m, e0.a);
                         hs_push(p.sink, b0 + g, k + 1, e1.m, e1.a);
@@ -284,19 +284,19 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
             }
             for (; i <= hi && i * n_w < N; i++) step_edge(i);
             emit(l);
-        } else if (OUT != HS_OUT_REDUCED) {
+        } else if ((OUT & 3) != HS_OUT_REDUCED) {
             emit(l);
         } else {
             tail = true;
         }
     }
     // With S unchanged over the skipped levels h_l = S c_l is monotone in l: testing the last level alone is enough.
-    if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
+    if ((OUT & 3) == HS_OUT_REDUCED && tail) emit(L - 1);
 
     if (OUT & HS_OUT_REDUCED) {
 #pragma unroll
         for (int q = 0; q < 4; q++) {
-            if (b0 + q < p.B && p.sink.cand) {
+            if (b0 + q < p.B && (OUT & HS_OUT_CAND)) {
 #pragma unroll
                 for (int k = 0; k < C; k++)
                     if (n0 + k < n_end) hs_push(p.sink, b0 + q, n0 + k, e[k][q].m, e[k][q].a);
@@ -460,7 +460,9 @@ int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
 {
     switch (p->out_mode) {
         case HS_OUT_FULL: return launch<L, HS_OUT_FULL>(p, buf, batch, ws, stream);
-        case HS_OUT_REDUCED: return launch<L, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
+        case HS_OUT_REDUCED:
+            if (buf.sink.cand) return launch<L, HS_OUT_REDUCED | HS_OUT_CAND>(p, buf, batch, ws, stream);
+            return launch<L, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
         default: return launch<L, HS_OUT_BOTH>(p, buf, batch, ws, stream);
     }
 }

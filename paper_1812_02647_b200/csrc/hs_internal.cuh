@@ -8,6 +8,7 @@
 #include "../../include/hs.h"
 
 #define HS_MAX_LEVELS 6
+#define HS_OUT_CAND 8   // internal OUT template bit: reduced output goes to the candidate sink (hs_execute_candidates)
 #define HS_HOST_LANES 3
 
 struct hs_plan {

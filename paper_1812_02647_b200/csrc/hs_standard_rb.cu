@@ -134,6 +134,7 @@ __device__ __forceinline__ void for_each_stage(F &f, std::integer_sequence<int, 
     (f(std::integral_constant<int, s>{}), ...);
 }
 
+template <bool CAND>
 __global__ void __launch_bounds__(kNT, kCtasPerSm)
 rb_kernel(const __grid_constant__ rb_params p)
 {
@@ -238,7 +239,7 @@ rb_kernel(const __grid_constant__ rb_params p)
 
         // ---- outputs of the tile: thread holds bins nw0 + 32 lane + [0, 32)
         const int64_t base = b * N + n0 + warp * 1024;
-        if (p.sink.cand) {                                               // hs_execute_candidates: no stores, rare appends
+        if constexpr (CAND) {   // hs_execute_candidates: no stores, rare appends
             float mm = m[0];
 #pragma unroll
             for (int r = 1; r < 32; r++) mm = fmaxf(mm, m[r]);
@@ -301,13 +302,15 @@ int hs_standard_rb_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch
     const size_t smem = (size_t)(kSlots * kSlot + (kNT / 32) * 32 * kOutRow) * sizeof(float);
     static bool configured = false;
     if (!configured) {
-        HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured = true;
     }
     const int64_t slots = (int64_t)p->sm_count * kCtasPerSm;
     const unsigned grid = (unsigned)(prm.tiles < slots ? prm.tiles : slots);
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, 256, stream));
-    rb_kernel<<<grid, kNT, smem, stream>>>(prm);
+    if (buf.sink.cand) rb_kernel<true><<<grid, kNT, smem, stream>>>(prm);
+    else rb_kernel<false><<<grid, kNT, smem, stream>>>(prm);
     HS_CUDA_OK(cudaGetLastError());
     return HS_OK;
 }

@@ -82,7 +82,7 @@ hs_std_tiled_kernel(const float *__restrict__ x, float *__restrict__ sums, float
                 e.level(l, S, plane0, N);
             }
             if (OUT & HS_OUT_REDUCED) {
-                if (sink.cand) {
+                if (OUT & HS_OUT_CAND) {
                     hs_push(sink, b, n, e.m, e.a);
                 } else {
                     hsptx::st_cs(vmax + b * (int64_t)N + n, e.m);
@@ -125,7 +125,9 @@ int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
 {
     switch (p->out_mode) {
         case HS_OUT_FULL: return launch<HMAX, HS_OUT_FULL>(p, buf, batch, stream);
-        case HS_OUT_REDUCED: return launch<HMAX, HS_OUT_REDUCED>(p, buf, batch, stream);
+        case HS_OUT_REDUCED:
+            if (buf.sink.cand) return launch<HMAX, HS_OUT_REDUCED | HS_OUT_CAND>(p, buf, batch, stream);
+            return launch<HMAX, HS_OUT_REDUCED>(p, buf, batch, stream);
         default: return launch<HMAX, HS_OUT_BOTH>(p, buf, batch, stream);
     }
 }

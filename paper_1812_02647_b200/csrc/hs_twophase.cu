@@ -274,7 +274,7 @@ __device__ __forceinline__ void phase2_round(const tp_params &p, const float *__
                 }
             }
             emit(l);
-        } else if (OUT != HS_OUT_REDUCED) {
+        } else if ((OUT & 3) != HS_OUT_REDUCED) {
             emit(l);
         } else {
             tail = true;
@@ -282,8 +282,8 @@ __device__ __forceinline__ void phase2_round(const tp_params &p, const float *__
     }
     // With S unchanged over the skipped levels, h_l = S c_l is monotone in l: for S >= 0 no later level can
     // exceed the running maximum, for S < 0 the last level is the largest.  Testing level L-1 alone is enough.
-    if (OUT == HS_OUT_REDUCED && tail) emit(L - 1);
-    if ((OUT & HS_OUT_REDUCED) && p.sink.cand) {
+    if ((OUT & 3) == HS_OUT_REDUCED && tail) emit(L - 1);
+    if ((OUT & HS_OUT_REDUCED) && (OUT & HS_OUT_CAND)) {
         if (fmaxf(fmaxf(e0.m, e1.m), fmaxf(e2.m, e3.m)) > p.sink.thr) {
             const int64_t b = row / p.N;
             hs_push(p.sink, b, n, e0.m, e0.a);
@@ -572,7 +572,9 @@ int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
 {
     switch (p->out_mode) {
         case HS_OUT_FULL: return launch<VARIANT, HMAX, HS_OUT_FULL>(p, buf, batch, ws, stream);
-        case HS_OUT_REDUCED: return launch<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
+        case HS_OUT_REDUCED:
+            if (buf.sink.cand) return launch<VARIANT, HMAX, HS_OUT_REDUCED | HS_OUT_CAND>(p, buf, batch, ws, stream);
+            return launch<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
         default: return launch<VARIANT, HMAX, HS_OUT_BOTH>(p, buf, batch, ws, stream);
     }
 }
