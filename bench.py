@@ -335,7 +335,10 @@ def main():
                                        "workspace_MiB": round(plans[v].workspace_bytes() / 2**20)}
     dominant = max(variants, key=lambda v: per_variant_ms[v])
     dom_algo = per_variant[dominant]["algo"]
-    roofline = {"bound": "hbm", "kernel": f"{dominant} ({dom_algo})", "achieved": per_variant[dominant]["eff_GBps"],
+    default_kernels = {"standard": "rb_kernel", "max": "gr_kernel", "freqbin": "il_persistent_kernel",
+                       "greedy": "hs_greedy_gather_kernel"}
+    kname = default_kernels[dominant] if (args.algo == "auto" and args.workload == "config2") else dom_algo
+    roofline = {"bound": "hbm", "kernel": f"{kname} ({dominant}, eq. {1 + VARIANTS.index(dominant) if dominant in VARIANTS else 0})", "achieved": per_variant[dominant]["eff_GBps"],
                 "peak": peak, "unit": "GB/s", "frac": per_variant[dominant]["eff_GBps"] / peak,
                 "traffic": ncu_traffic(dominant, args.workload, dom_algo),
                 "algorithmic_bytes_per_launch": bpb * batch * nbins, "peak_source": peak_src}
