@@ -13,13 +13,17 @@
 // Work items, handed out in order from one global counter, step s = 0, 1, ..:
 //     T(s):   copy 512 bins x 16 spectra of group s into its ring slot; bins n >= N/2 have no harmonic but the first
 //             in range (S_H(n) = x(n) for every H), so their outputs are emitted right here, in the natural layout;
-//     G(s-2): 128 (bins below N/8) or 512 bins x 16 spectra of the gather for group s-2 (bins below N/2 only), low
+//     G(s-1): 256 (bins below N/8) or 512 bins x 16 spectra of the gather for group s-1 (bins below N/2 only), low
 //             (= long) bins first;
-// T and G items of a step are interleaved in proportion, so that the HBM-bound copy and the L2/L1-bound gather overlap
-// on every SM.  A G item waits (acquire load on a per-group counter) until all T items of its group are done: those
-// were handed out a whole step earlier.  A T item waits until the gather of the group that used its ring slot last
-// (g - R, R = 4) is done: handed out at least a step earlier too.  Items only ever wait for items handed out EARLIER, and an
-// item is handed out to a CTA that is running, so the schedule cannot deadlock and needs no co-residency.
+// Within a step all T items come first, then all G items.  A G item waits (acquire load on a per-group counter) until all
+// T items of its group are done: those were handed out in the first half of the previous step.  A T item waits until the
+// gather of the group that used its ring slot last (g - R, R = 3) is done: handed out in the second half of step s - 2.
+// Every dependence therefore points at least a full step (~2.7 rounds of the resident CTAs) back and nothing waits, with a
+// ring of only 3 x 16 MiB = 48 MiB: proportional interleaving of the T and G items needed R = 4, lag 2 for that, and the
+// larger ring was written back to HBM almost entirely (4.30 -> 3.85 ms, profiles/r01_experiments.md).  CTAs drift apart
+// within a step, so the HBM-bound copies and the L2-bound gathers still overlap on the machine as a whole.  Items only
+// ever wait for items handed out EARLIER, and an item is handed out to a CTA that is running, so the schedule cannot
+// deadlock and needs no co-residency.
 //
 // Gather thread = (spectrum g of the group, C = 8 consecutive bins): 8 independent chains per thread hide Greedy's
 // serial dependence j -> address -> load, and the outputs of a thread are two float4 and two 4-byte stores.  Range
@@ -43,10 +47,10 @@ constexpr int kLPR = G / 4;                              // lanes per row of xT 
 constexpr int kWarpBins = (32 / kLPR) * C;              // bins per warp
 constexpr int kGTile = kWarps * kWarpBins;              // 256 bins per gather tile
 constexpr int kGSub = 2;                                // tiles per G item above the heavy region (bins >= N/8), 1 below
-constexpr int kLagDefault = 2;                          // the gather runs `lag` steps behind the copy
+constexpr int kLagDefault = 1;                          // the gather runs `lag` steps behind the copy
 constexpr int kTBins = 512 * 16 / G;                    // bins per T item (32 KiB of input)
 constexpr int kTStride = kTBins + 4;                    // shared-memory row stride (floats) of the copy tile
-constexpr int kMaxRing = 4;
+constexpr int kMaxRing = 3;
 
 struct il_params {
     const float *x;
@@ -56,7 +60,7 @@ struct il_params {
     uint8_t *amax;
     int *ctrl;          // [0] work counter, [1] error flag, [2..5] wait statistics, [16 + g] T items done, [16 + groups + g] G items done
     int64_t slot_words;
-    int N, B, groups, R, lag;
+    int N, B, groups, R, lag, order;
     hs_cand_sink sink;
     int nT, nG;         // items per group
     int nHeavy;         // the first nHeavy G items are single tiles (bins below ~N/8: 8 to 32 harmonics per bin)
@@ -341,7 +345,8 @@ il_persistent_kernel(const __grid_constant__ il_params p)
         if (threadIdx.x == 0) next = atomicAdd(queue, 1);               // in flight while this item runs
         const int s = item / per, r = item - s * per;
         // T and G items of a step interleaved in proportion nT : nG
-        const int t_before = (int)(((int64_t)r * p.nT) / per), t_after = (int)(((int64_t)(r + 1) * p.nT) / per);
+        const int t_before = p.order ? min(r, p.nT) : (int)(((int64_t)r * p.nT) / per);
+        const int t_after = p.order ? min(r + 1, p.nT) : (int)(((int64_t)(r + 1) * p.nT) / per);
         if (t_after > t_before) {                                       // ---- T item t_before of group s
             if (s < p.groups) {
                 float *xT = p.xT + (int64_t)(s % p.R) * p.slot_words;
@@ -436,6 +441,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.groups = s.groups;
     prm.R = s.R;
     prm.lag = s.lag;
+    prm.order = getenv("HS_IL_ORDER") ? atoi(getenv("HS_IL_ORDER")) : 1;
     prm.nT = s.nT;
     prm.nG = s.nG;
     prm.nHeavy = s.nHeavy;
