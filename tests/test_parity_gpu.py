@@ -344,3 +344,47 @@ def test_candidates_capacity_count_and_errors(hs, oracle):
     with pytest.raises(hs.HsError) as e:
         full.run_candidates(d_x, 3.0)
     assert e.value.code == hs.HS_ERR_INVALID_ARG
+
+
+# ---------------------------------------------------------------------------------------------------- guard bands
+@pytest.mark.parametrize("algo", ALGOS)
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_no_writes_outside_the_output_and_workspace_buffers(hs, variant, algo):
+    """Every output and the workspace sit between canary bands inside one allocation; after hs_execute (both output
+    modes at once) and hs_execute_candidates the bands are untouched.  (compute-sanitizer is not available on the box.)"""
+    G = 4096                                                      # guard elements on either side
+    for N, B in ((20000, 3), (1 << 15, 5), (4100, 2)):
+        x = (torch.empty((B, N), device="cuda").exponential_() - 1)
+        for out_mode in ("both", "reduced"):
+            plan = make_plan(hs, N, B, 32, variant, out_mode, algo)
+            L = plan.levels
+
+            def guarded(nelem, dtype, fill):
+                buf = torch.full((nelem + 2 * G,), fill, dtype=dtype, device="cuda")
+                return buf, buf[G:G + nelem]
+
+            sums_all, sums = guarded(B * L * N, torch.float32, -777.0)
+            vmax_all, vmax = guarded(B * N, torch.float32, -777.0)
+            amax_all, amax = guarded(B * N, torch.uint8, 0xAB)
+            ws_bytes = plan.workspace_bytes()
+            ws_all, ws = guarded(max(ws_bytes, 256), torch.uint8, 0xCD)
+            assert ws.data_ptr() % 256 == 0                       # (torch allocations are 512-byte aligned, G = 4096)
+            if ws_bytes:
+                plan.set_workspace(ws)
+            plan.hs_execute(x, sums.view(B, L, N) if out_mode == "both" else None, vmax.view(B, N), amax.view(B, N))
+            if out_mode == "reduced":
+                cand = torch.full((64 + 2 * G, 4), -5, dtype=torch.int32, device="cuda")
+                count = torch.zeros(1, dtype=torch.int64, device="cuda")
+                plan.hs_execute_candidates(x, 1.5, cand[G:G + 64], 64, count)
+            torch.cuda.synchronize()
+            what = f"{variant}/{algo}/{out_mode}/N={N}"
+            for name, whole, fill in (("sums", sums_all, -777.0), ("max", vmax_all, -777.0), ("argmax", amax_all, 0xAB),
+                                      ("workspace", ws_all, 0xCD)):
+                assert bool((whole[:G] == fill).all()) and bool((whole[-G:] == fill).all()), f"{what}: wrote outside {name}"
+            if out_mode == "reduced":
+                assert bool((cand[:G] == -5).all()) and bool((cand[G + 64:] == -5).all()), f"{what}: wrote outside the records"
+                assert int(count.item()) > 64                     # (more candidates than room: the rest must be dropped)
+            else:
+                assert bool((sums != -777.0).all()), f"{what}: a plane element was not written"
+            assert bool((vmax != -777.0).all()), f"{what}: a max element was not written"
+            plan.hs_destroy()
