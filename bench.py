@@ -372,41 +372,52 @@ def main():
     # ---- e2e: the same step through hs_execute_host with pinned host buffers -------------------------------------------
     e2e = None
     if not args.no_e2e:
-        slab = max(1, min(batch, (1 << 26) // nbins))          # 256 MiB of input per slab
-        h_x = torch.empty((batch, nbins), dtype=torch.float32, pin_memory=True)
-        h_x.copy_(x)
-        h_sums = torch.empty((batch, L, nbins), dtype=torch.float32, pin_memory=True) if sums is not None else None
-        h_max = torch.empty((batch, nbins), dtype=torch.float32, pin_memory=True) if vmax is not None else None
-        h_amax = torch.empty((batch, nbins), dtype=torch.uint8, pin_memory=True) if amax is not None else None
-        stagings = {}
-        for v in variants:
-            st = torch.empty(plans[v].host_staging_bytes(slab), dtype=torch.uint8, device=dev)
-            plans[v].set_host_staging(st, slab)
-            stagings[v] = st
-
-        def host_step():
+        ok, why = 1, ""
+        try:
+            slab = max(1, min(batch, (1 << 26) // nbins))          # 256 MiB of input per slab
+            h_x = torch.empty((batch, nbins), dtype=torch.float32, pin_memory=True)
+            h_x.copy_(x)
+            h_sums = torch.empty((batch, L, nbins), dtype=torch.float32, pin_memory=True) if sums is not None else None
+            h_max = torch.empty((batch, nbins), dtype=torch.float32, pin_memory=True) if vmax is not None else None
+            h_amax = torch.empty((batch, nbins), dtype=torch.uint8, pin_memory=True) if amax is not None else None
+            stagings = {}
             for v in variants:
-                plans[v].hs_execute_host(h_x, h_sums, h_max, h_amax, stream)
+                st = torch.empty(plans[v].host_staging_bytes(slab), dtype=torch.uint8, device=dev)
+                plans[v].set_host_staging(st, slab)
+                stagings[v] = st
+        except (RuntimeError, MemoryError) as exc:     # e.g. no room for the pinned host buffers: report, do not fail the line
+            ok, why = 0, str(exc).splitlines()[0][:200]
+        if world > 1:                                  # every rank takes the same branch (the timed part has a barrier)
+            flag = torch.tensor([ok], dtype=torch.int32, device=dev)
+            dist.all_reduce(flag, op=dist.ReduceOp.MIN)
+            ok = int(flag.item())
+        if not ok:
+            e2e = {"value": None, "unit": "bins/s", "unavailable": why or "another rank could not allocate its host buffers"}
+        else:
 
-        host_step()
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        t0 = time.perf_counter()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        for _ in range(args.e2e_steps):
+            def host_step():
+                for v in variants:
+                    plans[v].hs_execute_host(h_x, h_sums, h_max, h_amax, stream)
+
             host_step()
-        e1.record(stream)
-        torch.cuda.synchronize()
-        wall_ms = (time.perf_counter() - t0) * 1e3
-        e2e_ms = max_over_ranks_ms(max(e0.elapsed_time(e1), wall_ms), dist if world > 1 else None) / args.e2e_steps
-        h2d = len(variants) * batch * nbins * 4
-        d2h = len(variants) * batch * nbins * (bpb - 4)
-        e2e = {"value": bins_per_step / (e2e_ms * 1e-3), "unit": "bins/s", "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": args.e2e_steps,
-               "slab_spectra": slab, "checksum_max": float(h_max[0, :16].sum()) if h_max is not None else None}
-        del stagings
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+            t0 = time.perf_counter()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(args.e2e_steps):
+                host_step()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            wall_ms = (time.perf_counter() - t0) * 1e3
+            e2e_ms = max_over_ranks_ms(max(e0.elapsed_time(e1), wall_ms), dist if world > 1 else None) / args.e2e_steps
+            h2d = len(variants) * batch * nbins * 4
+            d2h = len(variants) * batch * nbins * (bpb - 4)
+            e2e = {"value": bins_per_step / (e2e_ms * 1e-3), "unit": "bins/s", "h2d_bytes_per_step": h2d,
+                   "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": args.e2e_steps,
+                   "slab_spectra": slab, "checksum_max": float(h_max[0, :16].sum()) if h_max is not None else None}
+            del stagings
 
     # ---- cpu_baseline: the oracle on a bounded sample of the same workload (rank 0, N = 1 only) ------------------------
     cpu = None
