@@ -4,7 +4,8 @@
 // Both variants have the form S_H(n) = sum_{i<=H} A_i(n) with a per-harmonic array that depends on x only:
 //     freq-bin  A_i(n) = x~(i n)                      the stride-i decimation of the spectrum
 //     Max       A_i(n) = max x~[i n .. i n + i - 1]   the maximum of the aligned block of size i
-// sum_{i=2..32} |A_i| = 3.06 N words.  One persistent, cooperatively launched kernel; CTA c belongs to group
+// sum_{i=2..32} |A_i| = 3.06 N words (at Hmax = 32 the arrays of sizes 2, 3, 4 are not kept: phase B takes those terms
+// from the spectrum itself, 1.98 N words remain -- `stored()` below).  One persistent, cooperatively launched kernel; CTA c belongs to group
 // c % groups with rank c / groups.  A group owns ONE workspace slot (3.06 N words) and walks through the spectra
 // g, g + groups, g + 2 groups, ..:
 //   phase A  the GS CTAs of the group share the spectrum's 4096-word chunks: chunk -> shared memory by one TMA bulk
@@ -48,6 +49,7 @@ constexpr size_t kL2Budget = (size_t)56 << 20;
 __host__ __device__ constexpr bool stored(int variant, int hyb, int i)
 {
     if (!hyb) return true;
+    if (hyb == 2) return i > 4;                  // grouped mode, trimmed: phase B takes sizes 2, 3, 4 from the spectrum
     if (variant == HS_MAX) return !(i == 2 || i == 3 || i == 4 || i == 6 || i == 8);
     return i > 8;
 }
@@ -186,17 +188,17 @@ __device__ __forceinline__ void max_pow2(const gr_params &p, const gr_smem &sm, 
     const float e32 = fmaxf(e16, __shfl_xor_sync(0xffffffffu, e16, 2));
     if (k >= p.N) continue;
     const bool whole = k + 8 <= p.N;                          // else exactly 4 bins are left (N % 4 == 0)
-    if (!HYB) {
+    if constexpr (stored(HS_MAX, HYB, 2)) {
         float *A2 = Ab + ((unsigned)p.lay.off[2] + (unsigned)(k >> 1));
         if (whole) *reinterpret_cast<float4 *>(A2) = make_float4(m0, m1, m2, m3);
         else *reinterpret_cast<float2 *>(A2) = make_float2(m0, m1);
-        if (HMAX >= 4) {
-            float *A4 = Ab + ((unsigned)p.lay.off[4] + (unsigned)(k >> 2));
-            if (whole) *reinterpret_cast<float2 *>(A4) = make_float2(q0, q1);
-            else A4[0] = q0;
-        }
-        if (HMAX >= 8) Ab[(unsigned)p.lay.off[8] + (unsigned)(k >> 3)] = e8;
     }
+    if constexpr (HMAX >= 4 && stored(HS_MAX, HYB, 4)) {
+        float *A4 = Ab + ((unsigned)p.lay.off[4] + (unsigned)(k >> 2));
+        if (whole) *reinterpret_cast<float2 *>(A4) = make_float2(q0, q1);
+        else A4[0] = q0;
+    }
+    if constexpr (HMAX >= 8 && stored(HS_MAX, HYB, 8)) Ab[(unsigned)p.lay.off[8] + (unsigned)(k >> 3)] = e8;
     if (HMAX >= 16 && (lane & 1) == 0) Ab[(unsigned)p.lay.off[16] + (unsigned)(k >> 4)] = e16;
     if (HMAX >= 32 && (lane & 3) == 0) Ab[(unsigned)p.lay.off[32] + (unsigned)(k >> 5)] = e32;
     }
@@ -214,17 +216,17 @@ __device__ __forceinline__ void dec_pow2(const gr_params &p, const gr_smem &sm, 
     const float4 u = *reinterpret_cast<const float4 *>(sm.raw + p0);
     const float4 w = *reinterpret_cast<const float4 *>(sm.raw + p0 + 4);
     const bool whole = k + 8 <= p.N;
-    if (!HYB) {
+    if constexpr (stored(HS_FREQBIN, HYB, 2)) {
         float *A2 = Ab + ((unsigned)p.lay.off[2] + (unsigned)(k >> 1));
         if (whole) *reinterpret_cast<float4 *>(A2) = make_float4(u.x, u.z, w.x, w.z);
         else *reinterpret_cast<float2 *>(A2) = make_float2(u.x, u.z);
-        if (HMAX >= 4) {
-            float *A4 = Ab + ((unsigned)p.lay.off[4] + (unsigned)(k >> 2));
-            if (whole) *reinterpret_cast<float2 *>(A4) = make_float2(u.x, w.x);
-            else A4[0] = u.x;
-        }
-        if (HMAX >= 8) Ab[(unsigned)p.lay.off[8] + (unsigned)(k >> 3)] = u.x;
     }
+    if constexpr (HMAX >= 4 && stored(HS_FREQBIN, HYB, 4)) {
+        float *A4 = Ab + ((unsigned)p.lay.off[4] + (unsigned)(k >> 2));
+        if (whole) *reinterpret_cast<float2 *>(A4) = make_float2(u.x, w.x);
+        else A4[0] = u.x;
+    }
+    if constexpr (HMAX >= 8 && stored(HS_FREQBIN, HYB, 8)) Ab[(unsigned)p.lay.off[8] + (unsigned)(k >> 3)] = u.x;
     if (HMAX >= 16 && (lane & 1) == 0) Ab[(unsigned)p.lay.off[16] + (unsigned)(k >> 4)] = u.x;
     if (HMAX >= 32 && (lane & 3) == 0) Ab[(unsigned)p.lay.off[32] + (unsigned)(k >> 5)] = u.x;
     }
@@ -457,7 +459,38 @@ __device__ __forceinline__ void phaseA_chunk(const gr_params &p, const gr_smem &
 // ---------------------------------------------------------------------------------------------- phase B
 // One warp tile = 128 consecutive outputs below n_split: lane holds bins n_first + 4 lane .. +3 as one float4.
 // The loads of a level are issued in batches of up to 8 float4 before they are consumed (memory-level parallelism).
-template <int L, int OUT>
+// Terms of harmonic I for the outputs n .. n + 3 straight from the spectrum: the window x[I n .. I n + 4 I) as I aligned
+// float4 loads (`whole`: warp-uniform, every element of the warp's windows in range), else element-wise with zero padding.
+template <int VARIANT, int I>
+__device__ __forceinline__ void add_from_x(float4 &S, const float *__restrict__ xrow, int n, int N, bool whole)
+{
+    float v[4 * I];
+    if (whole) {
+#pragma unroll
+        for (int q = 0; q < I; q++) {
+            const float4 t = __ldg(reinterpret_cast<const float4 *>(xrow + I * n) + q);
+            v[4 * q] = t.x, v[4 * q + 1] = t.y, v[4 * q + 2] = t.z, v[4 * q + 3] = t.w;
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4 * I; k++) v[k] = I * n + k < N ? __ldg(xrow + I * n + k) : 0.0f;   // zero padding (C5)
+    }
+    float t[4];
+#pragma unroll
+    for (int o = 0; o < 4; o++) {
+        t[o] = v[I * o];
+        if (VARIANT == HS_MAX) {
+#pragma unroll
+            for (int k = 1; k < I; k++) t[o] = fmaxf(t[o], v[I * o + k]);
+        }
+    }
+    S.x += t[0];
+    S.y += t[1];
+    S.z += t[2];
+    S.w += t[3];
+}
+
+template <int L, int OUT, int VARIANT = HS_MAX, int HYB = 0>
 __device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__restrict__ Ab, int64_t row, int n_first)
 {
     const int N = p.N;
@@ -484,7 +517,15 @@ __device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__r
         constexpr int kBatch = 8;
         const int lo = (1 << (l - 1)) + 1, hi = 1 << l;
         if ((int64_t)lo * n_first < N) {                           // warp-uniform: the level has a harmonic in range
-            if ((int64_t)hi * (n_first + kTileB) <= N) {           // warp-uniform: every element of the level in range
+            if (HYB == 2 && l <= 2) {                              // sizes 2, 3, 4 are not kept: straight from the spectrum
+                const float *__restrict__ xrow = p.x + row;
+                if (l == 1) {
+                    add_from_x<VARIANT, 2>(S, xrow, n, N, 2 * (n_first + kTileB) <= N);
+                } else {
+                    add_from_x<VARIANT, 3>(S, xrow, n, N, 3 * (n_first + kTileB) <= N);
+                    add_from_x<VARIANT, 4>(S, xrow, n, N, 4 * (n_first + kTileB) <= N);
+                }
+            } else if ((int64_t)hi * (n_first + kTileB) <= N) {    // warp-uniform: every element of the level in range
 #pragma unroll
                 for (int i0 = lo; i0 <= hi; i0 += kBatch) {
                     float4 v[kBatch];
@@ -544,7 +585,7 @@ struct gr_pos {
     int b, c;  // spectrum, chunk
 };
 
-template <int VARIANT, int HMAX, int OUT>
+template <int VARIANT, int HMAX, int OUT, int HYB>
 __global__ void __launch_bounds__(kThreads, 4)
 gr_kernel(const __grid_constant__ gr_params p)
 {
@@ -630,7 +671,7 @@ gr_kernel(const __grid_constant__ gr_params p)
             const int valid = min(kChunk + kHalo, N - k0);                // words the copy delivered (multiple of 4)
             for (int w = valid + threadIdx.x; w < kRaw; w += kThreads) sm.raw[w] = 0.0f;   // zero padding (C5)
             __syncthreads();
-            if (!(p.dbg & 1)) phaseA_chunk<VARIANT, HMAX, 0>(p, sm, Ab, k0);
+            if (!(p.dbg & 1)) phaseA_chunk<VARIANT, HMAX, HYB>(p, sm, Ab, k0);
             if (k0 >= p.n_split) emit_upper<L, OUT>(p, sm, (int64_t)b * N, k0);
             __syncthreads();                                              // raw/tables/bounds are reused
             tick(2);
@@ -653,7 +694,7 @@ gr_kernel(const __grid_constant__ gr_params p)
             j = __shfl_sync(0xffffffffu, j, 0);
             const int tile = rank + p.GS * j;
             if (tile >= p.ntiles || (p.dbg & 2)) break;
-            phaseB_tile<L, OUT>(p, Ab, row, tile * kTileB);
+            phaseB_tile<L, OUT, VARIANT, HYB>(p, Ab, row, tile * kTileB);
         }
         __syncthreads();                                                  // every load of the slot has returned
         tick(4);
@@ -672,11 +713,19 @@ struct gr_sched {
 
 constexpr int kCtasPerSm = 4;
 
+// Hmax = 32: the arrays of sizes 2, 3, 4 (1.08 N of the 3.06 N words) are not kept, phase B takes those terms from the
+// spectrum (HS_GR_HYB=0 keeps every array)
+int gr_hyb(const hs_plan *p)
+{
+    if (p->Hmax != 32) return 0;
+    return getenv("HS_GR_HYB") ? atoi(getenv("HS_GR_HYB")) : 2;   // measured: eq. 2 6.85 -> 6.72 ms, eq. 3 5.76 -> 4.96 ms
+}
+
 gr_sched make_sched(const hs_plan *p, int64_t batch)
 {
     gr_sched s{};
     const int N = (int)p->nbins;
-    s.lay = make_layout(N, p->Hmax);
+    s.lay = make_layout(N, p->Hmax, p->variant, gr_hyb(p));
     s.nchunks = (N + kChunk - 1) / kChunk;
     s.n_split = p->Hmax == 1 ? 0 : (int)(((int64_t)(N + 1) / 2 + kChunk - 1) / kChunk * kChunk);   // bins >= n_split: emitted by phase A
     s.ntiles = ((s.n_split < N ? s.n_split : N) + kTileB - 1) / kTileB;
@@ -703,8 +752,8 @@ size_t smem_bytes(int variant, int Hmax)
     return (size_t)((tabs ? 1 : 2) * kRaw + tabs * kTab) * sizeof(float);
 }
 
-template <int VARIANT, int HMAX, int OUT>
-int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+template <int VARIANT, int HMAX, int OUT, int HYB>
+int launch_hyb(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
     const gr_sched s = make_sched(p, batch);
     gr_params prm{};
@@ -724,7 +773,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.ntiles = s.ntiles;
     prm.n_split = s.n_split;
     prm.dbg = getenv("HS_GR_DBG") ? atoi(getenv("HS_GR_DBG")) : 0;
-    auto kern = gr_kernel<VARIANT, HMAX, OUT>;
+    auto kern = gr_kernel<VARIANT, HMAX, OUT, HYB>;
     const size_t smem = smem_bytes(VARIANT, HMAX);
     static bool configured = false;
     if (!configured) {
@@ -740,6 +789,15 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     HS_CUDA_OK(cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(kern), dim3((unsigned)(s.groups * s.GS)),
                                            dim3(kThreads), args, smem, stream));
     return HS_OK;
+}
+
+template <int VARIANT, int HMAX, int OUT>
+int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    if constexpr (HMAX == 32) {
+        if (gr_hyb(p) == 2) return launch_hyb<VARIANT, HMAX, OUT, 2>(p, buf, batch, ws, stream);
+    }
+    return launch_hyb<VARIANT, HMAX, OUT, 0>(p, buf, batch, ws, stream);
 }
 
 template <int VARIANT, int HMAX>
