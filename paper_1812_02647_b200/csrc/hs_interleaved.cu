@@ -13,7 +13,7 @@
 // Work items, handed out in order from one global counter, step s = 0, 1, ..:
 //     T(s):   copy 512 bins x 16 spectra of group s into its ring slot; bins n >= N/2 have no harmonic but the first
 //             in range (S_H(n) = x(n) for every H), so their outputs are emitted right here, in the natural layout;
-//     G(s-1): 256 (bins below N/8) or 512 bins x 16 spectra of the gather for group s-1 (bins below N/2 only), low
+//     G(s-1): 256 (bins below N/8) or 768 bins x 16 spectra of the gather for group s-1 (bins below N/2 only), low
 //             (= long) bins first;
 // Within a step all T items come first, then all G items.  A G item waits (acquire load on a per-group counter) until all
 // T items of its group are done: those were handed out in the first half of the previous step.  A T item waits until the
@@ -46,7 +46,8 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kLPR = G / 4;                              // lanes per row of xT (one float4 = 4 spectra each)
 constexpr int kWarpBins = (32 / kLPR) * C;              // bins per warp
 constexpr int kGTile = kWarps * kWarpBins;              // 256 bins per gather tile
-constexpr int kGSub = 2;                                // tiles per G item above the heavy region (bins >= N/8), 1 below
+constexpr int kGSub = 3;                                // tiles per G item above the heavy region (bins >= N/8), 1 below
+                                                        // (B200: 1 -> 4.03 ms, 2 -> 3.84, 3 -> 3.76, 4 -> 3.73 with waits, 8 -> 5.2)
 constexpr int kLagDefault = 1;                          // the gather runs `lag` steps behind the copy
 constexpr int kTBins = 512 * 16 / G;                    // bins per T item (32 KiB of input)
 constexpr int kTStride = kTBins + 4;                    // shared-memory row stride (floats) of the copy tile
