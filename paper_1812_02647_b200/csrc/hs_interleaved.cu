@@ -62,6 +62,7 @@ struct il_params {
     int *ctrl;          // [0] work counter, [1] error flag, [2..5] wait statistics, [16 + g] T items done, [16 + groups + g] G items done
     int64_t slot_words;
     int N, B, groups, R, lag, order;
+    int K;              // groups per step (order 1): short spectra need several groups for a step of a few rounds
     hs_cand_sink sink;
     int nT, nG;         // items per group
     int nHeavy;         // the first nHeavy G items are single tiles (bins below ~N/8: 8 to 32 harmonics per bin)
@@ -335,8 +336,8 @@ il_persistent_kernel(const __grid_constant__ il_params p)
     __shared__ int s_item;
     int *queue = p.ctrl, *err = p.ctrl + 1;
     int *doneT = p.ctrl + 16, *doneG = p.ctrl + 16 + p.groups;
-    const int per = p.nT + p.nG;
-    const int total = (p.groups + p.lag) * per;
+    const int per = p.nT + p.nG, per_step = p.K * per;
+    const int total = ((p.groups + p.K - 1) / p.K + p.lag) * per_step;
     int lastT = -1, lastG = -1;                                         // thread 0: groups already seen complete
     if (threadIdx.x == 0) s_item = atomicAdd(queue, 1);
     __syncthreads();
@@ -344,11 +345,24 @@ il_persistent_kernel(const __grid_constant__ il_params p)
     while (item < total) {
         int next = 0;
         if (threadIdx.x == 0) next = atomicAdd(queue, 1);               // in flight while this item runs
-        const int s = item / per, r = item - s * per;
-        // T and G items of a step interleaved in proportion nT : nG
-        const int t_before = p.order ? min(r, p.nT) : (int)(((int64_t)r * p.nT) / per);
-        const int t_after = p.order ? min(r + 1, p.nT) : (int)(((int64_t)(r + 1) * p.nT) / per);
-        if (t_after > t_before) {                                       // ---- T item t_before of group s
+        // step st = K groups: all their T items first, then the G items of the K groups of step st - lag (order 1);
+        // order 0 (K = 1): T and G items interleaved in proportion nT : nG
+        const int st = item / per_step, r = item - st * per_step;
+        bool isT;
+        int s, idx;                                                     // group and item index inside the group
+        if (p.order) {
+            isT = r < p.K * p.nT;
+            const int r2 = isT ? r : r - p.K * p.nT, n_per = isT ? p.nT : p.nG;
+            const int g = r2 / n_per;
+            idx = r2 - g * n_per;
+            s = (isT ? st : st - p.lag) * p.K + g;
+        } else {
+            const int t_before = (int)(((int64_t)r * p.nT) / per), t_after = (int)(((int64_t)(r + 1) * p.nT) / per);
+            isT = t_after > t_before;
+            idx = isT ? t_before : r - t_before;
+            s = isT ? st : st - p.lag;
+        }
+        if (isT) {                                                      // ---- T item idx of group s
             if (s < p.groups) {
                 float *xT = p.xT + (int64_t)(s % p.R) * p.slot_words;
                 if (threadIdx.x == 0 && s >= p.R && p.nG > 0 && lastG < s - p.R) {
@@ -356,22 +370,22 @@ il_persistent_kernel(const __grid_constant__ il_params p)
                     lastG = s - p.R;
                 }
                 __syncthreads();
-                copy_item<L, OUT>(p, tile, s, t_before * kTBins, xT);
+                copy_item<L, OUT>(p, tile, s, idx * kTBins, xT);
                 __syncthreads();                                        // all stores of the CTA are ordered before ...
                 if (threadIdx.x == 0) {
                     __threadfence();                                    // ... thread 0's release at gpu scope
                     atomicAdd(doneT + s, 1);
                 }
             }
-        } else if (s >= p.lag) {                                         // ---- G item (r - t_before) of group s - kLag
-            const int grp = s - p.lag;
+        } else if (s >= 0 && s < p.groups) {                            // ---- G item idx of group s
+            const int grp = s;
             const float *xT = p.xT + (int64_t)(grp % p.R) * p.slot_words;
             if (threadIdx.x == 0 && lastT < grp) {
                 wait_count(doneT + grp, p.nT, err, p.ctrl + 4);
                 lastT = grp;
             }
             __syncthreads();
-            const int q = r - t_before;
+            const int q = idx;
             if (q < p.nHeavy) {
                 gather_item<L, OUT>(p, grp, q * kGTile, xT);
             } else {
@@ -393,7 +407,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
 }
 
 struct il_sched {
-    int groups, R, lag, nT, nG, nHeavy, n_split;
+    int groups, R, lag, K, nT, nG, nHeavy, n_split;
     int64_t slot_words;
 };
 
@@ -406,7 +420,6 @@ il_sched make_sched(const hs_plan *p, int64_t batch)
     s.lag = kLagDefault;
     if (getenv("HS_IL_RING")) ring = atoi(getenv("HS_IL_RING"));
     if (getenv("HS_IL_LAG")) s.lag = atoi(getenv("HS_IL_LAG"));
-    s.R = s.groups < ring ? s.groups : ring;
     s.nT = (N + kTBins - 1) / kTBins;
     // bins n >= N/2 have S_H(n) = x(n): the T items emit them.  The split is a multiple of the T tile.
     const int half = (N + 1) / 2;
@@ -419,6 +432,15 @@ il_sched make_sched(const hs_plan *p, int64_t batch)
     if (s.nHeavy > tiles) s.nHeavy = tiles;
     s.nG = s.nHeavy + (tiles - s.nHeavy + kGSub - 1) / kGSub;
     s.slot_words = ((int64_t)N * G + 63) & ~(int64_t)63;
+    // groups per step: a step has to be ~2.6 rounds of the resident CTAs (2 per SM) or its dependences are exercised;
+    // one group of 2^18-bin spectra is that long, shorter spectra take several (the ring stays 48 MiB)
+    const int per = s.nT + s.nG;
+    int K = (int)((2.6 * 2 * p->sm_count + per / 2) / per);
+    if (getenv("HS_IL_K")) K = atoi(getenv("HS_IL_K"));
+    if (K < 1 || getenv("HS_IL_ORDER")) K = 1;
+    s.K = K;
+    ring *= K;
+    s.R = s.groups < ring ? s.groups : ring;
     return s;
 }
 
@@ -442,6 +464,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.groups = s.groups;
     prm.R = s.R;
     prm.lag = s.lag;
+    prm.K = s.K;
     prm.order = getenv("HS_IL_ORDER") ? atoi(getenv("HS_IL_ORDER")) : 1;
     prm.nT = s.nT;
     prm.nG = s.nG;
@@ -455,7 +478,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
         ctas_per_sm = occ > 0 ? occ : 1;
     }
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(s.groups), stream));
-    const int64_t total = (int64_t)(s.groups + s.lag) * (s.nT + s.nG);
+    const int64_t total = (int64_t)((s.groups + s.K - 1) / s.K + s.lag) * s.K * (s.nT + s.nG);
     const int64_t slots = (int64_t)p->sm_count * ctas_per_sm;
     kern<<<(unsigned)(total < slots ? total : slots), kThreads, 0, stream>>>(prm);
     HS_CUDA_OK(cudaGetLastError());
@@ -495,7 +518,7 @@ bool hs_interleaved_supported(const hs_plan *p)
     if (p->variant != HS_FREQBIN) return false;
     if (p->nbins > ((int64_t)1 << 18)) return false;
     const il_sched s = make_sched(p, p->batch);
-    return ((int64_t)s.groups + s.lag) * (s.nT + s.nG) < ((int64_t)1 << 30);
+    return ((int64_t)(s.groups + s.K - 1) / s.K + s.lag) * s.K * (s.nT + s.nG) < ((int64_t)1 << 30);
 }
 
 size_t hs_interleaved_workspace_bytes(const hs_plan *p, int64_t batch)
