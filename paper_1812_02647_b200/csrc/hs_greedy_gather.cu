@@ -60,22 +60,32 @@ __device__ __forceinline__ float max_window_rt(const float *__restrict__ w, int 
     }
 }
 
-template <int VARIANT, int L, int OUT, int Q>
+// SAME = false: the Q chains of a thread are the same bin of Q consecutive spectra.  SAME = true (long spectra, where Q
+// spectra in flight per CTA row would not fit L2): the Q chains are the bins n, n + 128, .., n + 128 (Q - 1) of ONE
+// spectrum; the warp-uniform bounds then span the CTA's Q blocks (safe: in range for the last block; any: for the first).
+template <int VARIANT, int L, int OUT, int Q, bool SAME>
 __global__ void __launch_bounds__(kThreads, Q >= 8 ? 8 : 12)
 hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
                         uint8_t *__restrict__ amax, int N, int batch, hs_cand_sink sink)
 {
-    const int n = blockIdx.x * kThreads + threadIdx.x;
-    const int n_lo = n & ~31;                      // first bin of this warp
+    const int n = blockIdx.x * (SAME ? kThreads * Q : kThreads) + threadIdx.x;
+    const int n_lo = n & ~31;                      // first bin of this warp (of its first block)
     if (n_lo >= N) return;
-    const bool valid = n < N;
-    const int nn = valid ? n : N - 1;              // lanes past the end shadow the last bin and store nothing
-    const int n_hi1 = min(n_lo + 32, N);           // one past the warp's last bin
+    constexpr int NB = SAME ? Q : 1;               // distinct bins per thread
+    bool valid[NB];
+    int nn[NB];
+#pragma unroll
+    for (int k = 0; k < NB; k++) {
+        valid[k] = n + k * kThreads < N;
+        nn[k] = valid[k] ? n + k * kThreads : N - 1;   // lanes past the end shadow the last bin and store nothing
+    }
+    const int n_hi1 = min(n_lo + (NB - 1) * kThreads + 32, N);   // one past the warp's last bin (of its last block)
     // Warp-uniform range tests (no divisions): harmonic i is in range for EVERY lane, neighbour included, iff
     // i * n_hi1 <= N; it is in range for SOME lane iff i * n_lo < N.
     // A thread runs the same bin of Q consecutive spectra side by side: the control flow depends on n only, so the Q
     // chains share every bound and give Q independent loads in flight (Greedy's chain is serial within a spectrum).
-    for (int b0 = blockIdx.y * Q; b0 < batch; b0 += gridDim.y * Q) {
+    constexpr int QS = SAME ? 1 : Q;               // spectra per thread
+    for (int b0 = blockIdx.y * QS; b0 < batch; b0 += gridDim.y * QS) {
         const float *__restrict__ xb[Q];
         bool live[Q];
         hs_emit<OUT> e[Q];
@@ -83,22 +93,24 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
         int j[Q];
 #pragma unroll
         for (int q = 0; q < Q; q++) {
-            live[q] = valid && b0 + q < batch;
-            xb[q] = x + (int64_t)min(b0 + q, batch - 1) * N;          // spectra past the batch shadow the last one
-            S[q] = __ldg(xb[q] + nn);
+            live[q] = valid[SAME ? q : 0] && b0 + (SAME ? 0 : q) < batch;
+            xb[q] = x + (int64_t)min(b0 + (SAME ? 0 : q), batch - 1) * N;   // spectra past the batch shadow the last one
+            S[q] = __ldg(xb[q] + nn[SAME ? q : 0]);
             j[q] = 0;
         }
         auto emit = [&](int l) {
 #pragma unroll
             for (int q = 0; q < Q; q++) {
                 const float h = S[q] * hs_norm(l);
-                if ((OUT & HS_OUT_FULL) && live[q]) hsptx::st_cs(sums + (((int64_t)(b0 + q) * L + l) * N + nn), h);
+                if ((OUT & HS_OUT_FULL) && live[q])
+                    hsptx::st_cs(sums + (((int64_t)(b0 + (SAME ? 0 : q)) * L + l) * N + nn[SAME ? q : 0]), h);
                 if (OUT & HS_OUT_REDUCED) e[q].reduce(l, h);
             }
         };
-        auto step = [&](int base, int i, bool safe) {   // harmonic i, i * n == base
+        auto step = [&](const int (&bases)[NB], int i, bool safe) {   // harmonic i, bases[k] == i * nn[k]
 #pragma unroll
             for (int q = 0; q < Q; q++) {
+                const int base = bases[SAME ? q : 0];
                 if (VARIANT == HS_FREQBIN) {        // eq. 3: x~(i n)
                     S[q] += (safe || base < N) ? __ldg(xb[q] + base) : 0.0f;
                 } else if (VARIANT == HS_MAX) {     // eq. 2 (Hmax <= 8): maximum of the aligned block x~[i n .. i n + i - 1]
@@ -126,13 +138,17 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
             const int lo = (1 << (l - 1)) + 1, hi = 1 << l;
             if (lo * n_lo < N) {                    // some harmonic of this level is in range for some lane
                 int i = lo;
-                int base = (lo - 1) * nn;           // (i - 1) * n
+                int base[NB];                       // (i - 1) * n
+#pragma unroll
+                for (int k = 0; k < NB; k++) base[k] = (lo - 1) * nn[k];
                 for (; i <= hi && i * n_hi1 <= N; i++) {
-                    base += nn;
+#pragma unroll
+                    for (int k = 0; k < NB; k++) base[k] += nn[k];
                     step(base, i, true);
                 }
                 for (; i <= hi && i * n_lo < N; i++) {
-                    base += nn;
+#pragma unroll
+                    for (int k = 0; k < NB; k++) base[k] += nn[k];
                     step(base, i, false);
                 }
                 emit(l);
@@ -148,32 +164,35 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
         if (OUT & HS_OUT_REDUCED) {
 #pragma unroll
             for (int q = 0; q < Q; q++) {
+                const int64_t bq = b0 + (SAME ? 0 : q);
+                const int nq = n + (SAME ? q * kThreads : 0);
                 if (live[q] && (OUT & HS_OUT_CAND)) {
-                    hs_push(sink, b0 + q, n, e[q].m, e[q].a);
+                    hs_push(sink, bq, nq, e[q].m, e[q].a);
                 } else if (live[q]) {
                     // (plain stores: measured 4 % faster here than the evict-first stores the other kernels use)
-                    vmax[(int64_t)(b0 + q) * N + n] = e[q].m;
-                    amax[(int64_t)(b0 + q) * N + n] = (uint8_t)e[q].a;
+                    vmax[bq * N + nq] = e[q].m;
+                    amax[bq * N + nq] = (uint8_t)e[q].a;
                 }
             }
         }
     }
 }
 
-template <int VARIANT, int L, int OUT, int Q>
+template <int VARIANT, int L, int OUT, int Q, bool SAME = false>
 int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     const int N = (int)p->nbins;
-    const int tiles = (N + kThreads - 1) / kThreads;
+    const int per_cta = SAME ? kThreads * Q : kThreads;
+    const int tiles = (N + per_cta - 1) / per_cta;
     const int64_t max_spectra = (int64_t)1 << 30;            // int b inside the kernel
     for (int64_t b0 = 0; b0 < batch; b0 += max_spectra) {
         const int64_t nb = (batch - b0 < max_spectra) ? batch - b0 : max_spectra;
         const int64_t off = b0 * (int64_t)N;
-        const int64_t gy = (nb + Q - 1) / Q;
+        const int64_t gy = SAME ? nb : (nb + Q - 1) / Q;
         const dim3 grid((unsigned)tiles, (unsigned)(gy < kGridY ? gy : kGridY), 1);
         hs_cand_sink sink = buf.sink;
         sink.b0 += (int)b0;
-        hs_greedy_gather_kernel<VARIANT, L, OUT, Q><<<grid, kThreads, 0, stream>>>(
+        hs_greedy_gather_kernel<VARIANT, L, OUT, Q, SAME><<<grid, kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
             buf.amax ? buf.amax + off : nullptr, N, (int)nb, sink);
         HS_CUDA_OK(cudaGetLastError());
@@ -181,13 +200,15 @@ int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_
     return HS_OK;
 }
 
-// Spectra side by side per thread: 8 while 8 spectra (and what is in flight around them) stay in L2; long spectra run
+// Spectra side by side per thread: 8 while 8 spectra (and what is in flight around them) stay in L2; longer spectra run
 // fewer at a time so that the gathers of all harmonics of a spectrum still hit L2 (2^22 bins = 16 MiB per spectrum).
 template <int VARIANT, int L, int OUT>
 int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
+    // spectra of more than 2^22 bins (32 MiB and up): 8 bin blocks of ONE spectrum per thread instead of 8 spectra
+    // (B200, 2^30 bins in all, 2^23-bin spectra: eq. 3 Hmax 2 2.11 -> 1.70 ms, Hmax 32 8.16 -> 6.08 ms; eq. 4 9.21 -> 7.42 ms)
+    if (p->nbins > ((int64_t)1 << 22)) return launch_q<VARIANT, L, OUT, kSpectraPerCta, true>(p, buf, batch, stream);
     if (L >= 5) {                                                  // (with few harmonics the loads in flight matter more)
-        if (p->nbins > ((int64_t)1 << 22)) return launch_q<VARIANT, L, OUT, 1>(p, buf, batch, stream);
         if (p->nbins > ((int64_t)1 << 20)) return launch_q<VARIANT, L, OUT, 2>(p, buf, batch, stream);
     }
     return launch_q<VARIANT, L, OUT, kSpectraPerCta>(p, buf, batch, stream);
