@@ -54,9 +54,10 @@ enum hs_algo {
     HS_ALGO_AUTO = 0,
     HS_ALGO_DIRECT = 1, /* one thread per output bin, loads straight from global memory; needs no workspace;
                            every variant; kept as the simple on-device reference                              */
-    HS_ALGO_TILED = 2,  /* the tuned kernels: eq. 1 windows staged in shared memory by TMA;
-                           eq. 2 two-phase through a workspace; eqs. 3-4 gather from a spectrum-interleaved copy of
-                           16 spectra at a time that stays in L2 (workspace)                                        */
+    HS_ALGO_TILED = 2,  /* the tuned kernels: eq. 1 register-blocked with TMA-streamed windows
+                           (workspace: a tile counter); eq. 2 grouped two-phase through L2-resident workspace slots;
+                           eq. 3 gather from a spectrum-interleaved copy of 16 spectra at a time (workspace ring);
+                           eq. 4, and eqs. 2-3 where those do not apply, the range-skipping gather                    */
     HS_ALGO_TWOPHASE = 3, /* eqs. 2-3 only: the two-phase kernel (for eq. 2 the same as HS_ALGO_TILED)              */
     HS_ALGO_GATHER = 4,   /* eqs. 3-4 only: the range-skipping gather straight from x (no workspace); what
                              HS_ALGO_TILED itself uses for spectra too long for the interleaved group copy           */
