@@ -207,7 +207,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
 {
     // spectra of more than 2^22 bins (32 MiB and up): 8 bin blocks of ONE spectrum per thread instead of 8 spectra
     // (B200, 2^30 bins in all, 2^23-bin spectra: eq. 3 Hmax 2 2.11 -> 1.70 ms, Hmax 32 8.16 -> 6.08 ms; eq. 4 9.21 -> 7.42 ms)
-    if (p->nbins > ((int64_t)1 << 22) || (L <= 2 && p->nbins >= 8192))   // (also with at most two harmonics: 5 - 8 % faster)
+    if (p->nbins > ((int64_t)1 << 22) || (L <= 2 && VARIANT != HS_MAX && p->nbins >= 8192))   // (eqs. 3-4 with two harmonics: 5 - 8 % faster)
         return launch_q<VARIANT, L, OUT, kSpectraPerCta, true>(p, buf, batch, stream);
     if (L >= 5) {                                                  // (with few harmonics the loads in flight matter more)
         if (p->nbins > ((int64_t)1 << 20)) return launch_q<VARIANT, L, OUT, 2>(p, buf, batch, stream);
