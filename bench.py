@@ -49,7 +49,7 @@ def parse():
     ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS))
     ap.add_argument("--batch", type=int, default=0, help="override the batch (non-headline; recorded in config)")
     ap.add_argument("--variants", default=",".join(VARIANTS))
-    ap.add_argument("--algo", default="auto", choices=["auto", "direct", "tiled", "twophase", "gather", "grouped", "streamed"])
+    ap.add_argument("--algo", default="auto", choices=["auto", "direct", "tiled", "twophase", "gather", "grouped"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="budget of the cpu_baseline leg")
@@ -274,7 +274,7 @@ def main():
     plans = {}
     for v in variants:
         p = hs.hs_plan_create(nbins, batch, 32, v, out_mode)
-        ok = not (args.algo in ("twophase", "grouped", "streamed") and v not in ("max", "freqbin")) and not (args.algo == "gather" and v not in ("freqbin", "greedy"))
+        ok = not (args.algo in ("twophase", "grouped") and v not in ("max", "freqbin")) and not (args.algo == "gather" and v not in ("freqbin", "greedy"))
         p.set_algo(args.algo if ok else "auto")
         p.ensure_workspace(dev)
         plans[v] = p

@@ -47,7 +47,9 @@ enum hs_status {
     HS_ERR_MISALIGNED = 3,   /* a base pointer is not 16-byte aligned                                   */
     HS_ERR_UNSUPPORTED = 4,  /* no CUDA device of compute capability 10.x is current                    */
     HS_ERR_WORKSPACE = 5,    /* the chosen algorithm needs a workspace that was not set or is too small */
-    HS_ERR_CUDA = 6          /* a CUDA runtime call or kernel launch failed                             */
+    HS_ERR_CUDA = 6,         /* a CUDA runtime call or kernel launch failed                             */
+    HS_ERR_DEVICE_TIMEOUT = 7 /* hs_plan_device_status: a kernel of the last execute gave up waiting for another
+                                 thread block (its outputs are then not valid)                          */
 };
 /* Kernel family.  HS_ALGO_AUTO picks the fastest one that is valid for the plan. */
 enum hs_algo {
@@ -61,12 +63,9 @@ enum hs_algo {
     HS_ALGO_TWOPHASE = 3, /* eqs. 2-3 only: the two-phase kernel (for eq. 2 the same as HS_ALGO_TILED)              */
     HS_ALGO_GATHER = 4,   /* eqs. 3-4 only: the range-skipping gather straight from x (no workspace); what
                              HS_ALGO_TILED itself uses for spectra too long for the interleaved group copy           */
-    HS_ALGO_GROUPED = 5,  /* eqs. 2-3 only: two phases per spectrum by a static group of co-resident CTAs, the
+    HS_ALGO_GROUPED = 5   /* eqs. 2-3 only, Hmax >= 2, nbins <= 2^23: two phases per spectrum by a static group of co-resident CTAs, the
                              per-harmonic arrays of a spectrum live in one L2-resident workspace slot per group
                              (cooperative launch)                                                                   */
-    HS_ALGO_STREAMED = 6  /* eqs. 2-3, Hmax 16 or 32: two plain kernels (per-harmonic arrays of the large block sizes
-                             only, written to and read back from a workspace of one slot per spectrum; the small
-                             sizes are evaluated from the spectrum itself); any spectrum length                     */
 };
 
 /*
@@ -75,10 +74,13 @@ enum hs_algo {
  * PAPER.md:17-46).
  *   nbins    bins per spectrum, 4 <= nbins <= 2^25 and nbins % 4 == 0 (16-byte rows for vector/bulk copies; bin indices
  *            up to 32*nbins+32 are int32)
- *   batch    number of spectra, 1 <= batch, batch*nbins <= 2^40
+ *   batch    number of spectra, 1 <= batch <= 2^31 - 1 (spectrum indices, also hs_candidate.spectrum, are int32),
+ *            batch*nbins <= 2^40
  *   Hmax     largest number of harmonics, one of 1,2,4,8,16,32
  *   variant  enum hs_variant;  out_mode  enum hs_out_mode
- * Does no device work.  Returns NULL on error: HS_ERR_INVALID_ARG (checked first), HS_ERR_UNSUPPORTED, HS_ERR_CUDA.
+ * Does no device work.  The plan belongs to the CUDA device that is current at the call: executing it with another
+ * device current fails with HS_ERR_INVALID_ARG.
+ * Returns NULL on error: HS_ERR_INVALID_ARG (checked first), HS_ERR_UNSUPPORTED, HS_ERR_CUDA.
  */
 hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode);
 
@@ -112,6 +114,17 @@ size_t hs_plan_workspace_bytes(const hs_plan *plan);     /* device scratch the r
 int hs_plan_set_workspace(hs_plan *plan, void *d_ws, size_t bytes);
 /* Number of kernel launches (memset nodes included) one hs_execute of this plan enqueues; -1 if plan is NULL. */
 int hs_plan_launches(const hs_plan *plan);
+/*
+ * hs_plan_device_status — SYNCHRONISES `stream`, then reads back the error word of the control block(s) the plan's last
+ * hs_execute / hs_execute_candidates / hs_execute_host launched with.  The persistent kernels (HS_ALGO_TILED for eqs. 2-4,
+ * HS_ALGO_GROUPED) hand work between thread blocks through counters in the workspace; a thread block that polls such a
+ * counter more than a bounded number of times (a scheduling bug, or a debugger / time-slicing stall of seconds) sets
+ * the error word and carries on, so that the GPU cannot hang: the outputs of that execute are then NOT valid.
+ * Returns HS_OK, HS_ERR_DEVICE_TIMEOUT, or HS_ERR_CUDA if the synchronisation / copy failed.  Plans whose kernels do
+ * not synchronise between thread blocks always return HS_OK (after synchronising).  Call it before trusting outputs
+ * in tests and benchmarks; hs_execute itself never synchronises.
+ */
+int hs_plan_device_status(const hs_plan *plan, void *stream);
 
 /*
  * hs_execute_host — the same transform with HOST buffers (pinned memory recommended): h_x, h_sums, h_max, h_argmax

@@ -9,16 +9,19 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libhs.so")
+# HS_LIBRARY names another build of the same sources in this directory (libhs_tuning.so: the -DHS_TUNING build used by
+# the builder's sweeps and the forced-timeout test); the default is the product library.
+LIB_PATH = os.path.join(_HERE, os.path.basename(os.environ.get("HS_LIBRARY", "libhs.so")))
 
 HS_STANDARD, HS_MAX, HS_FREQBIN, HS_GREEDY = 0, 1, 2, 3
 HS_OUT_FULL, HS_OUT_REDUCED, HS_OUT_BOTH = 1, 2, 3
-HS_ALGO_AUTO, HS_ALGO_DIRECT, HS_ALGO_TILED, HS_ALGO_TWOPHASE, HS_ALGO_GATHER, HS_ALGO_GROUPED, HS_ALGO_STREAMED = 0, 1, 2, 3, 4, 5, 6
-HS_OK, HS_ERR_INVALID_ARG, HS_ERR_NULL_POINTER, HS_ERR_MISALIGNED, HS_ERR_UNSUPPORTED, HS_ERR_WORKSPACE, HS_ERR_CUDA = range(7)
+HS_ALGO_AUTO, HS_ALGO_DIRECT, HS_ALGO_TILED, HS_ALGO_TWOPHASE, HS_ALGO_GATHER, HS_ALGO_GROUPED = 0, 1, 2, 3, 4, 5
+(HS_OK, HS_ERR_INVALID_ARG, HS_ERR_NULL_POINTER, HS_ERR_MISALIGNED, HS_ERR_UNSUPPORTED, HS_ERR_WORKSPACE, HS_ERR_CUDA,
+ HS_ERR_DEVICE_TIMEOUT) = range(8)
 VARIANTS = {"standard": HS_STANDARD, "max": HS_MAX, "freqbin": HS_FREQBIN, "greedy": HS_GREEDY}
 OUT_MODES = {"full": HS_OUT_FULL, "reduced": HS_OUT_REDUCED, "both": HS_OUT_BOTH}
 ALGOS = {"auto": HS_ALGO_AUTO, "direct": HS_ALGO_DIRECT, "tiled": HS_ALGO_TILED, "twophase": HS_ALGO_TWOPHASE,
-         "gather": HS_ALGO_GATHER, "grouped": HS_ALGO_GROUPED, "streamed": HS_ALGO_STREAMED}
+         "gather": HS_ALGO_GATHER, "grouped": HS_ALGO_GROUPED}
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build the CUDA library with `python -m paper_1812_02647_b200.build` "
@@ -39,6 +42,7 @@ _SIGS = {
     "hs_plan_workspace_bytes": ([_p], _sz),
     "hs_plan_set_workspace": ([_p, _p, _sz], _int),
     "hs_plan_launches": ([_p], _int),
+    "hs_plan_device_status": ([_p, _p], _int),
     "hs_execute_host": ([_p, _p, _p, _p, _p, _p], _int),
     "hs_plan_host_staging_bytes": ([_p, _i64], _sz),
     "hs_plan_set_host_staging": ([_p, _p, _sz, _i64], _int),
@@ -121,6 +125,11 @@ class Plan:
 
     def launches(self) -> int:
         return lib.hs_plan_launches(self.handle)
+
+    def device_status(self, stream=None) -> int:
+        """hs_plan_device_status: synchronises the stream; raises HsError(HS_ERR_DEVICE_TIMEOUT) if a kernel gave up a wait."""
+        _check(lib.hs_plan_device_status(self.handle, _stream(stream)), "hs_plan_device_status")
+        return HS_OK
 
     def hs_execute(self, d_x, d_sums=None, d_max=None, d_argmax=None, stream=None):
         _check(lib.hs_execute(self.handle, _ptr(d_x), _ptr(d_sums), _ptr(d_max), _ptr(d_argmax), _stream(stream)),

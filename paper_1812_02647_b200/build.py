@@ -1,8 +1,11 @@
 """Builds paper_1812_02647_b200/libhs.so (the C-ABI library of include/hs.h) in-tree with nvcc for sm_100a.
 
-    python -m paper_1812_02647_b200.build [--force]
+    python -m paper_1812_02647_b200.build [--force] [-v] [--tuning]
 
 One object per .cu (compiled in parallel), then one shared library.  nvcc cross-compiles without a GPU.
+--tuning builds libhs_tuning.so instead: the same sources with -DHS_TUNING, the only build in which the kernels'
+schedule parameters (ring sizes, lags, spin limit) can be overridden through HS_* environment variables.  The product
+library reads no environment variable; the tuning build serves the builder's sweeps and the forced-timeout test.
 """
 from __future__ import annotations
 
@@ -16,6 +19,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libhs.so")
+LIB_TUNING = os.path.join(HERE, "libhs_tuning.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC,-Wall,-Wextra", "--expt-relaxed-constexpr"]
@@ -29,10 +33,10 @@ def _stale(target, sources):
     return (not os.path.exists(target)) or any(os.path.getmtime(s) > os.path.getmtime(target) for s in sources)
 
 
-def _compile(src, verbose):
-    obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
+def _compile(src, verbose, tuning=False):
+    obj = os.path.join(OBJ, os.path.basename(src)[:-3] + (".tuning.o" if tuning else ".o"))
     if _stale(obj, [src] + _deps()):
-        cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+        cmd = [NVCC] + FLAGS + (["-DHS_TUNING"] if tuning else []) + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")
@@ -41,20 +45,22 @@ def _compile(src, verbose):
     return obj
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, tuning: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
+    lib = LIB_TUNING if tuning else LIB
     srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
     if force:
-        for f in glob.glob(os.path.join(OBJ, "*.o")):
-            os.remove(f)
-    with concurrent.futures.ThreadPoolExecutor(max_workers=min(8, len(srcs))) as ex:
-        objs = list(ex.map(lambda s: _compile(s, verbose), srcs))
-    if force or _stale(LIB, objs):
-        tmp = LIB + f".tmp{os.getpid()}"
+        for f in glob.glob(os.path.join(OBJ, "*.tuning.o" if tuning else "*.o")):
+            if tuning or not f.endswith(".tuning.o"):
+                os.remove(f)
+    with concurrent.futures.ThreadPoolExecutor(max_workers=min(os.cpu_count() or 4, len(srcs))) as ex:
+        objs = list(ex.map(lambda s: _compile(s, verbose, tuning), srcs))
+    if force or _stale(lib, objs):
+        tmp = lib + f".tmp{os.getpid()}"
         subprocess.check_call([NVCC, "-shared", "-o", tmp] + objs)
-        os.replace(tmp, LIB)
-    return LIB
+        os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, tuning="--tuning" in sys.argv))

@@ -26,11 +26,39 @@ void resolve_algo(hs_plan *p)
 {
     if (p->algo_req == HS_ALGO_DIRECT) p->algo = HS_ALGO_DIRECT;
     else if (p->algo_req == HS_ALGO_TILED || p->algo_req == HS_ALGO_TWOPHASE || p->algo_req == HS_ALGO_GATHER ||
-             p->algo_req == HS_ALGO_GROUPED || p->algo_req == HS_ALGO_STREAMED)
+             p->algo_req == HS_ALGO_GROUPED)
         p->algo = HS_ALGO_TILED;
     else p->algo = hs_tiled_supported(p) ? HS_ALGO_TILED : HS_ALGO_DIRECT;
+    // the workspace and the host staging were sized for the previous algorithm: both have to be set again
     p->ws = nullptr;
     p->ws_bytes = 0;
+    p->staging = nullptr;
+    p->staging_bytes = 0;
+    p->slab = 0;
+    p->n_last_ctrl = 0;
+}
+
+// the plan's device must be current (function attributes, occupancy and the SM count are per device)
+int check_device(const hs_plan *p)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        HS_FAIL(HS_ERR_CUDA);
+    }
+    if (dev != p->device) HS_FAIL(HS_ERR_INVALID_ARG);
+    return HS_OK;
+}
+
+// remember which control block a launch used (hs_plan_device_status)
+void note_ctrl(const hs_plan *p, const void *ws, bool first)
+{
+    if (first) p->n_last_ctrl = 0;
+    if (ws && p->algo == HS_ALGO_TILED && hs_tiled_has_ctrl(p) && p->n_last_ctrl < HS_HOST_LANES) {
+        for (int i = 0; i < p->n_last_ctrl; i++)
+            if (p->last_ctrl[i] == ws) return;
+        p->last_ctrl[p->n_last_ctrl++] = ws;
+    }
 }
 
 int check_buffers(const hs_plan *p, const void *x, const void *sums, const void *vmax, const void *amax)
@@ -44,7 +72,7 @@ int check_buffers(const hs_plan *p, const void *x, const void *sums, const void 
 
 int launch_family(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
-    if (p->algo == HS_ALGO_TILED && !buf.jdbg) return hs_launch_tiled(p, buf, batch, ws, stream);
+    if (p->algo == HS_ALGO_TILED) return hs_launch_tiled(p, buf, batch, ws, stream);
     return hs_launch_direct(p, buf, batch, ws, stream);
 }
 
@@ -84,18 +112,19 @@ const char *hs_error_string(int code)
         case HS_ERR_UNSUPPORTED: return "no CUDA device of compute capability 10.x (sm_100) is current";
         case HS_ERR_WORKSPACE: return "workspace or staging buffer missing or too small";
         case HS_ERR_CUDA: return "CUDA runtime call or kernel launch failed";
+        case HS_ERR_DEVICE_TIMEOUT: return "a kernel gave up waiting for another thread block: outputs are not valid";
         default: return "unknown hs_status code";
     }
 }
 
-const char *hs_version(void) { return "hs 0.1 (sm_100a)"; }
+const char *hs_version(void) { return "hs 0.2 (sm_100a)"; }
 
 hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode)
 {
     const int L = levels_of(Hmax);
     if (nbins < 4 || nbins > ((int64_t)1 << 25) || (nbins % 4) != 0 || batch < 1 || L < 0 ||
         variant < HS_STANDARD || variant > HS_GREEDY || out_mode < HS_OUT_FULL || out_mode > HS_OUT_BOTH ||
-        batch > ((int64_t)1 << 40) / nbins) {
+        batch > ((int64_t)1 << 40) / nbins || batch > (int64_t)0x7fffffff) {
         hs_set_error(HS_ERR_INVALID_ARG);
         return nullptr;
     }
@@ -128,6 +157,7 @@ hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int
     p->variant = variant;
     p->out_mode = out_mode;
     p->algo_req = HS_ALGO_AUTO;
+    p->device = dev;
     p->sm_count = sms;
     p->smem_optin = (size_t)smem;
     p->staging = nullptr;
@@ -159,17 +189,15 @@ int hs_plan_algo(const hs_plan *p) { return p ? p->algo : -1; }
 int hs_plan_set_algo(hs_plan *p, int algo)
 {
     if (!p) HS_FAIL(HS_ERR_NULL_POINTER);
-    if (algo < HS_ALGO_AUTO || algo > HS_ALGO_STREAMED) HS_FAIL(HS_ERR_INVALID_ARG);
-    if ((algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GROUPED || algo == HS_ALGO_STREAMED) && p->variant != HS_MAX &&
-        p->variant != HS_FREQBIN)
+    if (algo < HS_ALGO_AUTO || algo > HS_ALGO_GROUPED) HS_FAIL(HS_ERR_INVALID_ARG);
+    if ((algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GROUPED) && p->variant != HS_MAX && p->variant != HS_FREQBIN)
         HS_FAIL(HS_ERR_INVALID_ARG);
     if (algo == HS_ALGO_GATHER && p->variant != HS_GREEDY && p->variant != HS_FREQBIN &&
         !(p->variant == HS_MAX && p->Hmax <= 4))
         HS_FAIL(HS_ERR_INVALID_ARG);
     const int before = p->algo_req;
     p->algo_req = algo;
-    if ((algo == HS_ALGO_TILED || algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GATHER || algo == HS_ALGO_GROUPED ||
-         algo == HS_ALGO_STREAMED) &&
+    if ((algo == HS_ALGO_TILED || algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GATHER || algo == HS_ALGO_GROUPED) &&
         !hs_tiled_supported(p)) {
         p->algo_req = before;
         HS_FAIL(HS_ERR_INVALID_ARG);
@@ -212,11 +240,13 @@ int hs_plan_launches(const hs_plan *p)
 
 int hs_execute(const hs_plan *p, const float *d_x, float *d_sums, float *d_max, uint8_t *d_argmax, void *stream)
 {
-    const int rc = check_buffers(p, d_x, d_sums, d_max, d_argmax);
+    int rc = check_buffers(p, d_x, d_sums, d_max, d_argmax);
     if (rc != HS_OK) return rc;
+    if ((rc = check_device(p)) != HS_OK) return rc;
     if (hs_plan_workspace_bytes(p) > 0 && (!p->ws || p->ws_bytes < hs_plan_workspace_bytes(p))) HS_FAIL(HS_ERR_WORKSPACE);
+    note_ctrl(p, p->ws, true);
     hs_buffers buf{d_x, (p->out_mode & HS_OUT_FULL) ? d_sums : nullptr, (p->out_mode & HS_OUT_REDUCED) ? d_max : nullptr,
-                   (p->out_mode & HS_OUT_REDUCED) ? d_argmax : nullptr, nullptr};
+                   (p->out_mode & HS_OUT_REDUCED) ? d_argmax : nullptr, nullptr, {}};
     return launch_family(p, buf, p->batch, p->ws, static_cast<cudaStream_t>(stream));
 }
 
@@ -226,7 +256,10 @@ int hs_execute_candidates(const hs_plan *p, const float *d_x, float threshold, h
     if (!p || !d_x || !d_count || (!d_cand && capacity > 0)) HS_FAIL(HS_ERR_NULL_POINTER);
     if (p->out_mode != HS_OUT_REDUCED || capacity < 0 || !(threshold == threshold)) HS_FAIL(HS_ERR_INVALID_ARG);
     if (!aligned(d_x, 16) || !aligned(d_cand, 16) || !aligned(d_count, 8)) HS_FAIL(HS_ERR_MISALIGNED);
+    const int rcd = check_device(p);
+    if (rcd != HS_OK) return rcd;
     if (hs_plan_workspace_bytes(p) > 0 && (!p->ws || p->ws_bytes < hs_plan_workspace_bytes(p))) HS_FAIL(HS_ERR_WORKSPACE);
+    note_ctrl(p, p->ws, true);
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     HS_CUDA_OK(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s));
     hs_buffers buf{d_x, nullptr, nullptr, nullptr, nullptr, {}};
@@ -245,8 +278,25 @@ int hs_debug_greedy_paths(const hs_plan *p, const float *d_x, uint8_t *d_j, void
     if (!p || !d_x || !d_j) HS_FAIL(HS_ERR_NULL_POINTER);
     if (p->variant != HS_GREEDY) HS_FAIL(HS_ERR_INVALID_ARG);
     if (!aligned(d_x, 16) || !aligned(d_j, 16)) HS_FAIL(HS_ERR_MISALIGNED);
-    hs_buffers buf{d_x, nullptr, nullptr, nullptr, d_j};
-    return hs_launch_direct(p, buf, p->batch, nullptr, static_cast<cudaStream_t>(stream));
+    const int rcd = check_device(p);
+    if (rcd != HS_OK) return rcd;
+    if (hs_plan_workspace_bytes(p) > 0 && (!p->ws || p->ws_bytes < hs_plan_workspace_bytes(p))) HS_FAIL(HS_ERR_WORKSPACE);
+    note_ctrl(p, p->ws, true);
+    // the plan's own kernel family in its own launch configuration, writing j instead of the outputs
+    hs_buffers buf{d_x, nullptr, nullptr, nullptr, d_j, {}};
+    return launch_family(p, buf, p->batch, p->ws, static_cast<cudaStream_t>(stream));
+}
+
+int hs_plan_device_status(const hs_plan *p, void *stream)
+{
+    if (!p) HS_FAIL(HS_ERR_NULL_POINTER);
+    HS_CUDA_OK(cudaStreamSynchronize(static_cast<cudaStream_t>(stream)));
+    for (int i = 0; i < p->n_last_ctrl; i++) {
+        int words[4] = {0, 0, 0, 0};
+        HS_CUDA_OK(cudaMemcpy(words, p->last_ctrl[i], sizeof(words), cudaMemcpyDeviceToHost));
+        if (words[HS_CTRL_ERROR] != 0) HS_FAIL(HS_ERR_DEVICE_TIMEOUT);
+    }
+    return HS_OK;
 }
 
 size_t hs_plan_host_staging_bytes(const hs_plan *p, int64_t slab)
@@ -281,8 +331,12 @@ int hs_execute_host(hs_plan *p, const float *h_x, float *h_sums, float *h_max, u
     if ((p->out_mode & HS_OUT_FULL) && !h_sums) HS_FAIL(HS_ERR_NULL_POINTER);
     if ((p->out_mode & HS_OUT_REDUCED) && (!h_max || !h_argmax)) HS_FAIL(HS_ERR_NULL_POINTER);
     if (!p->lanes_ready || !p->staging) HS_FAIL(HS_ERR_WORKSPACE);
+    const int rcd = check_device(p);
+    if (rcd != HS_OK) return rcd;
     cudaStream_t user = static_cast<cudaStream_t>(stream);
     const slab_layout lay = layout_of(p, p->slab);
+    if (p->staging_bytes < lay.total * HS_HOST_LANES) HS_FAIL(HS_ERR_WORKSPACE);   // (sized for another algorithm)
+    p->n_last_ctrl = 0;
     const int64_t N = p->nbins;
     HS_CUDA_OK(cudaEventRecord(p->fork, user));
     for (int i = 0; i < HS_HOST_LANES; i++) HS_CUDA_OK(cudaStreamWaitEvent(p->lane_stream[i], p->fork, 0));
@@ -298,7 +352,8 @@ int hs_execute_host(hs_plan *p, const float *h_x, float *h_sums, float *h_max, u
         void *dws = lay.ws ? base + lay.x + lay.sums + lay.vmax + lay.amax : nullptr;
         cudaStream_t s = p->lane_stream[lane];
         HS_CUDA_OK(cudaMemcpyAsync(dx, h_x + (size_t)b0 * N, bins * 4, cudaMemcpyHostToDevice, s));
-        hs_buffers buf{dx, dsums, dmax, damax, nullptr};
+        hs_buffers buf{dx, dsums, dmax, damax, nullptr, {}};
+        note_ctrl(p, dws, false);
         const int rc = launch_family(p, buf, nb, dws, s);
         if (rc != HS_OK) return rc;
         if (dsums)

@@ -63,10 +63,11 @@ __device__ __forceinline__ float max_window_rt(const float *__restrict__ w, int 
 // SAME = false: the Q chains of a thread are the same bin of Q consecutive spectra.  SAME = true (long spectra, where Q
 // spectra in flight per CTA row would not fit L2): the Q chains are the bins n, n + 128, .., n + 128 (Q - 1) of ONE
 // spectrum; the warp-uniform bounds then span the CTA's Q blocks (safe: in range for the last block; any: for the first).
-template <int VARIANT, int L, int OUT, int Q, bool SAME>
+// JDBG (hs_debug_greedy_paths, eq. 4 only, OUT = 0): the drift j after each level goes to jdbg[b][l][n] instead of the outputs.
+template <int VARIANT, int L, int OUT, int Q, bool SAME, bool JDBG = false>
 __global__ void __launch_bounds__(kThreads, Q >= 8 ? 8 : 12)
 hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
-                        uint8_t *__restrict__ amax, int N, int batch, hs_cand_sink sink)
+                        uint8_t *__restrict__ amax, uint8_t *__restrict__ jdbg, int N, int batch, hs_cand_sink sink)
 {
     const int n = blockIdx.x * (SAME ? kThreads * Q : kThreads) + threadIdx.x;
     const int n_lo = n & ~31;                      // first bin of this warp (of its first block)
@@ -105,6 +106,8 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
                 if ((OUT & HS_OUT_FULL) && live[q])
                     hsptx::st_cs(sums + (((int64_t)(b0 + (SAME ? 0 : q)) * L + l) * N + nn[SAME ? q : 0]), h);
                 if (OUT & HS_OUT_REDUCED) e[q].reduce(l, h);
+                if (JDBG && live[q])
+                    jdbg[((int64_t)(b0 + (SAME ? 0 : q)) * L + l) * N + nn[SAME ? q : 0]] = (uint8_t)j[q];
             }
         };
         auto step = [&](const int (&bases)[NB], int i, bool safe) {   // harmonic i, bases[k] == i * nn[k]
@@ -152,7 +155,7 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
                     step(base, i, false);
                 }
                 emit(l);
-            } else if ((OUT & 3) != HS_OUT_REDUCED) {
+            } else if ((OUT & 3) != HS_OUT_REDUCED || JDBG) {
                 emit(l);
             } else {
                 tail = true;
@@ -178,7 +181,7 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
     }
 }
 
-template <int VARIANT, int L, int OUT, int Q, bool SAME = false>
+template <int VARIANT, int L, int OUT, int Q, bool SAME = false, bool JDBG = false>
 int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     const int N = (int)p->nbins;
@@ -192,9 +195,9 @@ int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_
         const dim3 grid((unsigned)tiles, (unsigned)(gy < kGridY ? gy : kGridY), 1);
         hs_cand_sink sink = buf.sink;
         sink.b0 += (int)b0;
-        hs_greedy_gather_kernel<VARIANT, L, OUT, Q, SAME><<<grid, kThreads, 0, stream>>>(
+        hs_greedy_gather_kernel<VARIANT, L, OUT, Q, SAME, JDBG><<<grid, kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
-            buf.amax ? buf.amax + off : nullptr, N, (int)nb, sink);
+            buf.amax ? buf.amax + off : nullptr, buf.jdbg ? buf.jdbg + off * L : nullptr, N, (int)nb, sink);
         HS_CUDA_OK(cudaGetLastError());
     }
     return HS_OK;
@@ -202,22 +205,25 @@ int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_
 
 // Spectra side by side per thread: 8 while 8 spectra (and what is in flight around them) stay in L2; longer spectra run
 // fewer at a time so that the gathers of all harmonics of a spectrum still hit L2 (2^22 bins = 16 MiB per spectrum).
-template <int VARIANT, int L, int OUT>
+template <int VARIANT, int L, int OUT, bool JDBG = false>
 int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     // spectra of more than 2^22 bins (32 MiB and up): 8 bin blocks of ONE spectrum per thread instead of 8 spectra
     // (B200, 2^30 bins in all, 2^23-bin spectra: eq. 3 Hmax 2 2.11 -> 1.70 ms, Hmax 32 8.16 -> 6.08 ms; eq. 4 9.21 -> 7.42 ms)
     if (p->nbins > ((int64_t)1 << 22) || (L <= 2 && VARIANT != HS_MAX && p->nbins >= 8192))   // (eqs. 3-4 with two harmonics: 5 - 8 % faster)
-        return launch_q<VARIANT, L, OUT, kSpectraPerCta, true>(p, buf, batch, stream);
+        return launch_q<VARIANT, L, OUT, kSpectraPerCta, true, JDBG>(p, buf, batch, stream);
     if (L >= 5) {                                                  // (with few harmonics the loads in flight matter more)
-        if (p->nbins > ((int64_t)1 << 20)) return launch_q<VARIANT, L, OUT, 2>(p, buf, batch, stream);
+        if (p->nbins > ((int64_t)1 << 20)) return launch_q<VARIANT, L, OUT, 2, false, JDBG>(p, buf, batch, stream);
     }
-    return launch_q<VARIANT, L, OUT, kSpectraPerCta>(p, buf, batch, stream);
+    return launch_q<VARIANT, L, OUT, kSpectraPerCta, false, JDBG>(p, buf, batch, stream);
 }
 
 template <int VARIANT, int L>
 int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
+    if constexpr (VARIANT == HS_GREEDY) {                          // the same kernel and launch shape, j instead of the outputs
+        if (buf.jdbg) return launch<VARIANT, L, 0, true>(p, buf, batch, stream);
+    }
     switch (p->out_mode) {
         case HS_OUT_FULL: return launch<VARIANT, L, HS_OUT_FULL>(p, buf, batch, stream);
         case HS_OUT_REDUCED:

@@ -26,11 +26,11 @@
 // words is conflict-free for odd j; size 2j is the union of an aligned pair of j-blocks: one shuffle-xor.
 // A chunk owns the super-blocks (size j K_j, K_j the largest power of two with j K_j <= Hmax) that START inside it and
 // reads a 32-word halo for those that run past its end.
-#include <cstdlib>
 #include <utility>
 
 #include "hs_internal.cuh"
 #include "hs_ptx.cuh"
+#include "hs_sync.cuh"
 
 namespace {
 
@@ -43,15 +43,14 @@ constexpr int kTab = kChunk + kHalo;      // table entries per width
 constexpr int kTileB = 128;               // phase-B outputs per warp tile (float4 per lane)
 constexpr size_t kL2Budget = (size_t)56 << 20;
 
-// Which per-harmonic arrays A_i exist.  HYB = 0 (grouped mode): every i = 2..Hmax.  HYB = 1 (streamed mode, below): the
-// small sizes are evaluated by phase B straight from the spectrum (a window of i words per output costs as much HBM
-// traffic as writing and re-reading A_i while i is small), so Max keeps only i not in {2, 3, 4, 6, 8} and freq-bin only i > 8.
+// Which per-harmonic arrays A_i exist.  HYB = 0: every i = 2..Hmax.  HYB = 2 (Hmax >= 8): the sizes 2, 3, 4 are evaluated
+// by phase B straight from the spectrum (a window of i words per output costs no more L2 traffic than writing and
+// re-reading A_i while i is small, and the slot shrinks from 3.06 N to 1.98 N words).
 __host__ __device__ constexpr bool stored(int variant, int hyb, int i)
 {
+    (void)variant;
     if (!hyb) return true;
-    if (hyb == 2) return i > 4;                  // grouped mode, trimmed: phase B takes sizes 2, 3, 4 from the spectrum
-    if (variant == HS_MAX) return !(i == 2 || i == 3 || i == 4 || i == 6 || i == 8);
-    return i > 8;
+    return i > 4;                                // hyb == 2: phase B takes sizes 2, 3, 4 from the spectrum
 }
 
 struct gr_layout {
@@ -80,7 +79,8 @@ struct gr_params {
     float *sums;
     float *vmax;
     uint8_t *amax;
-    int *ctrl;       // [0] error flag, [1] spinning waits, [2] spins; [32 + 64 g] phase-A arrivals, [64 + 64 g] phase-B arrivals of group g
+    int *ctrl;       // control block (hs_internal.cuh): [1] error flag, [2] spinning waits, [3] polls; [32 + 64 g] phase-A
+                     // arrivals, [64 + 64 g] phase-B arrivals of group g
     gr_layout lay;
     int N, B;
     int groups, GS;  // number of groups, CTAs per group
@@ -88,7 +88,7 @@ struct gr_params {
     int ntiles;      // phase-B warp tiles per spectrum: they cover the bins below n_split
     int n_split;     // multiple of kChunk, >= N/2: the outputs of bins n >= n_split are emitted by phase A
     hs_cand_sink sink;
-    int dbg;         // experiments only: 1 skip phase A, 2 skip phase B, 4 skip the barriers
+    unsigned spin_limit;
 };
 
 constexpr int chain_len(int j, int hmax)  // K_j: largest power of two with j*K <= hmax
@@ -99,33 +99,7 @@ constexpr int chain_len(int j, int hmax)  // K_j: largest power of two with j*K 
 }
 constexpr int ilog2c(int v) { return v <= 1 ? 0 : 1 + ilog2c(v >> 1); }
 
-__device__ __forceinline__ int ld_acquire(const int *p)
-{
-    int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void red_release_add(int *p, int v)
-{
-    asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
-// thread 0 only: wait until *cnt >= target (bounded: a bug must not hang the GPU; the error flag makes it visible)
-__device__ __forceinline__ void wait_count(const int *cnt, int target, int *ctrl)
-{
-    unsigned spins = 0;
-    while (ld_acquire(cnt) < target) {
-        __nanosleep(32);
-        if (++spins > (1u << 22) || (spins & 1023u) == 0 && ld_acquire(ctrl) != 0) {
-            atomicExch(ctrl, 1);
-            break;
-        }
-    }
-    if (spins) {
-        atomicAdd(ctrl + 1, 1);
-        atomicAdd(ctrl + 2, (int)(spins > 0xffffu ? 0xffffu : spins));
-    }
-}
+using hssync::red_release_add;
 
 // ---------------------------------------------------------------------------------------------- phase A
 // Shared-memory view of one chunk: raw[kRaw] holds x[k0 .. k0 + kChunk + kHalo) (zero beyond the spectrum, C5) and
@@ -632,14 +606,6 @@ gr_kernel(const __grid_constant__ gr_params p)
     };
 
     gr_pos cur{grp, rank};
-    long long t_acc[6] = {0, 0, 0, 0, 0, 0}, t_last = clock64();     // dbg & 8: cycles per stage, thread 0
-    auto tick = [&](int k) {
-        if ((p.dbg & 8) && threadIdx.x == 0) {
-            const long long t = clock64();
-            t_acc[k] += t - t_last;
-            t_last = t;
-        }
-    };
     int buf = 0;
     uint32_t parity = 0u;                                                 // bit `buf`: phase of that buffer's barrier
     if (threadIdx.x == 0 && cur.b < p.B) issue(cur, 0);
@@ -648,10 +614,9 @@ gr_kernel(const __grid_constant__ gr_params p)
         const int b = cur.b;
         // the slot is free once every CTA of the group has finished phase B of the previous spectrum
         if (it > 0) {
-            if (threadIdx.x == 0 && !(p.dbg & 4)) wait_count(cntB, p.GS * it, p.ctrl);
+            if (threadIdx.x == 0) hssync::wait_count(cntB, p.GS * it, p.ctrl, p.ctrl + HS_CTRL_STATS, p.spin_limit);
             __syncthreads();
         }
-        tick(0);
         // ---- phase A: this CTA's chunks of spectrum b
         while (cur.b == b) {
             const gr_pos nxt = advance(cur);
@@ -666,15 +631,13 @@ gr_kernel(const __grid_constant__ gr_params p)
             }
             hsptx::mbar_wait(&bar[buf], (parity >> buf) & 1u);
             parity ^= 1u << buf;
-            tick(1);
             sm.raw = dyn + buf * kRaw;
             const int valid = min(kChunk + kHalo, N - k0);                // words the copy delivered (multiple of 4)
             for (int w = valid + threadIdx.x; w < kRaw; w += kThreads) sm.raw[w] = 0.0f;   // zero padding (C5)
             __syncthreads();
-            if (!(p.dbg & 1)) phaseA_chunk<VARIANT, HMAX, HYB>(p, sm, Ab, k0);
+            phaseA_chunk<VARIANT, HMAX, HYB>(p, sm, Ab, k0);
             if (k0 >= p.n_split) emit_upper<L, OUT>(p, sm, (int64_t)b * N, k0);
             __syncthreads();                                              // raw/tables/bounds are reused
-            tick(2);
             if (kRawBufs == 1 && threadIdx.x == 0 && nxt.b < p.B) issue(nxt, 0);
             cur = nxt;
             if (kRawBufs == 2) buf ^= 1;
@@ -682,10 +645,9 @@ gr_kernel(const __grid_constant__ gr_params p)
         if (threadIdx.x == 0) {
             s_next = 0;
             red_release_add(cntA, 1);                                     // (cumulative: ordered after the CTA's stores)
-            if (!(p.dbg & 4)) wait_count(cntA, p.GS * (it + 1), p.ctrl);
+            hssync::wait_count(cntA, p.GS * (it + 1), p.ctrl, p.ctrl + HS_CTRL_STATS, p.spin_limit);
         }
         __syncthreads();
-        tick(3);
         // ---- phase B: the group's warps share the tiles; a CTA takes tiles rank, rank + GS, .. heavy (low n) first
         const int64_t row = (int64_t)b * N;
         for (;;) {
@@ -693,16 +655,12 @@ gr_kernel(const __grid_constant__ gr_params p)
             if ((threadIdx.x & 31) == 0) j = atomicAdd(&s_next, 1);
             j = __shfl_sync(0xffffffffu, j, 0);
             const int tile = rank + p.GS * j;
-            if (tile >= p.ntiles || (p.dbg & 2)) break;
+            if (tile >= p.ntiles) break;
             phaseB_tile<L, OUT, VARIANT, HYB>(p, Ab, row, tile * kTileB);
         }
         __syncthreads();                                                  // every load of the slot has returned
-        tick(4);
         if (threadIdx.x == 0) red_release_add(cntB, 1);
     }
-    if ((p.dbg & 8) && threadIdx.x == 0)
-        for (int k = 0; k < 5; k++)
-            atomicAdd(reinterpret_cast<unsigned long long *>(p.ctrl + 8) + k, (unsigned long long)t_acc[k]);
 }
 
 // ---------------------------------------------------------------------------------------------- host side
@@ -718,7 +676,7 @@ constexpr int kCtasPerSm = 4;
 int gr_hyb(const hs_plan *p)
 {
     if (p->Hmax < 8) return 0;
-    return getenv("HS_GR_HYB") ? atoi(getenv("HS_GR_HYB")) : 2;   // measured: eq. 2 6.85 -> 6.72 ms, eq. 3 5.76 -> 4.96 ms
+    return hs_knob("HS_GR_HYB", 2);   // measured: eq. 2 6.85 -> 6.72 ms, eq. 3 5.76 -> 4.96 ms
 }
 
 gr_sched make_sched(const hs_plan *p, int64_t batch)
@@ -734,7 +692,7 @@ gr_sched make_sched(const hs_plan *p, int64_t batch)
     // CTAs per group: the smallest power of two for which all the groups' slots together fit the L2 budget
     int GS = 1;
     while ((slots / GS) * slot_bytes > kL2Budget + kL2Budget / 8 && GS * 2 <= slots) GS *= 2;
-    if (getenv("HS_GR_GS")) GS = atoi(getenv("HS_GR_GS"));
+    if (hs_knob("HS_GR_GS", 0) > 0) GS = hs_knob("HS_GR_GS", 0);
     while (GS > 1 && (GS > s.nchunks || GS > s.ntiles)) GS /= 2;
     int64_t groups = slots / GS;
     if (groups > batch) groups = batch;
@@ -772,17 +730,14 @@ int launch_hyb(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws,
     prm.nchunks = s.nchunks;
     prm.ntiles = s.ntiles;
     prm.n_split = s.n_split;
-    prm.dbg = getenv("HS_GR_DBG") ? atoi(getenv("HS_GR_DBG")) : 0;
+    prm.spin_limit = hs_spin_limit();
     auto kern = gr_kernel<VARIANT, HMAX, OUT, HYB>;
     const size_t smem = smem_bytes(VARIANT, HMAX);
-    static bool configured = false;
-    if (!configured) {
-        HS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        int occ = 0;
-        HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, smem));
-        if (occ < kCtasPerSm) HS_FAIL(HS_ERR_CUDA);       // the groups' CTAs wait for one another: all must be resident
-        configured = true;
-    }
+    // (function attributes are per device: set on every launch rather than once per process)
+    HS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, smem));
+    if (occ < kCtasPerSm) HS_FAIL(HS_ERR_CUDA);           // the groups' CTAs wait for one another: all must be resident
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(s.groups), stream));
     void *args[] = {&prm};
     // cooperative launch: fails instead of deadlocking if the grid cannot be co-resident
@@ -824,248 +779,13 @@ int by_hmax(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cu
     }
 }
 
-
-// ====================================================================================================================
-// Streamed mode (HS_ALGO_STREAMED): the same two phases as two PLAIN kernels per wave of spectra, no inter-CTA
-// synchronisation at all.  Phase A (one CTA per 4096-word chunk, the code above with HYB = 1) keeps only the arrays
-// phase B cannot get cheaply from the spectrum itself; phase B (one thread per output bin below n_split) evaluates the
-// small block sizes / strides straight from x -- a window of i consecutive words per output, read with the widest
-// aligned vector load -- and adds the kept A_i with unit stride.  Per bin at Hmax = 32 the kept arrays are 1.68 (Max)
-// or 1.34 (freq-bin) words instead of 3.06, and every kernel is a plain stream over its inputs, so the mode works for
-// any spectrum length and is bound by HBM (x twice, the kept arrays written and read once, the outputs once:
-// 26.4 B/bin for Max) when a wave's arrays do not fit L2, and by L2 when they do (wave = HS_ST_WAVE spectra).
-constexpr bool st_hmax_ok(int hmax) { return hmax == 16 || hmax == 32; }
-
-template <int VARIANT, int HMAX, int OUT>
-__global__ void __launch_bounds__(kThreads, 4)
-st_phaseA_kernel(const __grid_constant__ gr_params p, int b0)
-{
-    constexpr int L = ilog2c(HMAX) + 1;
-    constexpr bool kTables = VARIANT == HS_MAX && HMAX >= 16;
-    extern __shared__ __align__(128) float dyn[];
-    __shared__ __align__(8) uint64_t bar;
-    __shared__ int2 s_bounds[33];
-    const int b = b0 + blockIdx.y, k0 = blockIdx.x * kChunk, N = p.N;
-    gr_smem sm;
-    sm.raw = dyn;
-    sm.T8 = dyn + kRaw;
-    sm.T16 = sm.T8 + (kTables && HMAX >= 32 ? kTab : 0);
-    sm.bounds = s_bounds;
-    const int valid = min(kChunk + kHalo, N - k0);                       // words of the spectrum in chunk + halo (multiple of 4)
-    if (threadIdx.x == 0) {
-        hsptx::mbar_init(&bar, 1);
-        hsptx::mbar_fence_init();
-        hsptx::mbar_arrive_expect_tx(&bar, (uint32_t)valid * 4u);
-        hsptx::bulk_g2s(dyn, p.x + (int64_t)b * N + k0, (uint32_t)valid * 4u, &bar);
-    }
-    if (threadIdx.x >= 3 && threadIdx.x <= HMAX) {
-        // entries of size i owned by the chunk: those whose super-block (i K words) starts inside it
-        const int i = threadIdx.x, K = VARIANT == HS_MAX ? chain_len(i, HMAX) : 1, sb = i * K;
-        const int first = K * ((k0 + sb - 1) / sb), last = K * ((k0 + kChunk + sb - 1) / sb);
-        const int lenK = (p.lay.len[i] + K - 1) / K * K;
-        s_bounds[i] = make_int2(first, min(last, lenK));
-    }
-    for (int w = valid + threadIdx.x; w < kRaw; w += kThreads) dyn[w] = 0.0f;   // zero padding (C5); disjoint from the copy
-    __syncthreads();                                                       // barrier initialised, bounds and padding visible
-    hsptx::mbar_wait(&bar, 0u);
-    float *__restrict__ Ab = p.A + (int64_t)(b % p.groups) * p.lay.slot_words;
-    phaseA_chunk<VARIANT, HMAX, 1>(p, sm, Ab, k0);
-    if (k0 >= p.n_split) emit_upper<L, OUT>(p, sm, (int64_t)b * N, k0);
-}
-
-// term of harmonic I at bin n, every element in range: the maximum of x[I n .. I n + I - 1] (Max) or x[I n] (freq-bin)
-template <int VARIANT, int I>
-__device__ __forceinline__ float st_term_safe(const float *__restrict__ xb, int n)
-{
-    const float *__restrict__ w = xb + (int64_t)I * n;
-    if (VARIANT == HS_FREQBIN) return __ldg(w);
-    if constexpr (I % 4 == 0) {
-        float m = 0.f;
-#pragma unroll
-        for (int q = 0; q < I / 4; q++) {
-            const float4 u = __ldg(reinterpret_cast<const float4 *>(w) + q);
-            const float t = fmaxf(fmaxf(u.x, u.y), fmaxf(u.z, u.w));
-            m = q == 0 ? t : fmaxf(m, t);
-        }
-        return m;
-    } else if constexpr (I % 2 == 0) {
-        float m = 0.f;
-#pragma unroll
-        for (int q = 0; q < I / 2; q++) {
-            const float2 u = __ldg(reinterpret_cast<const float2 *>(w) + q);
-            const float t = fmaxf(u.x, u.y);
-            m = q == 0 ? t : fmaxf(m, t);
-        }
-        return m;
-    } else {
-        float m = __ldg(w);
-#pragma unroll
-        for (int q = 1; q < I; q++) m = fmaxf(m, __ldg(w + q));
-        return m;
-    }
-}
-// the same with zero padding beyond the spectrum (C5: the zeros take part in the maximum)
-template <int VARIANT, int I>
-__device__ __forceinline__ float st_term_edge(const float *__restrict__ xb, int n, int N)
-{
-    const int k = I * n;
-    if (VARIANT == HS_FREQBIN) return k < N ? __ldg(xb + k) : 0.f;
-    float m = k < N ? __ldg(xb + k) : 0.f;
-#pragma unroll
-    for (int q = 1; q < I; q++) m = fmaxf(m, k + q < N ? __ldg(xb + k + q) : 0.f);
-    return m;
-}
-
-constexpr int kStThreads = 256;
-
-template <class F, int... k>
-__device__ __forceinline__ void st_static_for(F &f, std::integer_sequence<int, k...>)
-{
-    (f(std::integral_constant<int, k>{}), ...);
-}
-
-template <int VARIANT, int HMAX, int OUT>
-__global__ void __launch_bounds__(kStThreads)
-st_phaseB_kernel(const __grid_constant__ gr_params p, int b0)
-{
-    constexpr int L = ilog2c(HMAX) + 1;
-    const int N = p.N, b = b0 + blockIdx.y;
-    const int n_end = min(N, p.n_split);                               // bins [n_end, N) were emitted by phase A
-    const int n = blockIdx.x * kStThreads + threadIdx.x;
-    const int n_lo = n & ~31;                                          // first bin of the warp
-    if (n_lo >= n_end) return;
-    const bool live = n < n_end;
-    const int nn = live ? n : n_end - 1;                               // lanes past the end shadow the last bin, store nothing
-    const int n_hi1 = min(n_lo + 32, n_end);                           // one past the warp's last bin
-    const float *__restrict__ xb = p.x + (int64_t)b * N;
-    const float *__restrict__ An = p.A + (int64_t)(b % p.groups) * p.lay.slot_words + nn;   // A_i[n] = An[off_i]
-    float S = __ldg(xb + nn);
-    hs_emit<OUT> e;
-    float *plane0 = (OUT & HS_OUT_FULL) ? p.sums + ((int64_t)b * L * N + nn) : nullptr;
-    auto emit = [&](int l) {
-        const float h = S * hs_norm(l);
-        if ((OUT & HS_OUT_FULL) && live) hsptx::st_cs(plane0 + (int64_t)l * N, h);
-        if (OUT & HS_OUT_REDUCED) e.reduce(l, h);
-    };
-    emit(0);
-    bool tail = false;
-    auto level = [&](auto lc) {
-        constexpr int l = decltype(lc)::value + 1, lo = (1 << (l - 1)) + 1, hi = 1 << l;
-        if ((int64_t)lo * n_lo < N) {                                  // warp-uniform: the level has a harmonic in range
-            auto harmonic = [&](auto ic) {
-                constexpr int i = decltype(ic)::value + lo;
-                if ((int64_t)i * n_hi1 <= N) {                         // warp-uniform: in range for every lane
-                    if constexpr (stored(VARIANT, 1, i)) S += __ldg(An + p.lay.off[i]);
-                    else S += st_term_safe<VARIANT, i>(xb, nn);
-                } else if ((int64_t)i * n_lo < N) {                    // warp-uniform: in range for some lane
-                    if constexpr (stored(VARIANT, 1, i)) S += nn < p.lay.len[i] ? __ldg(An + p.lay.off[i]) : 0.f;
-                    else S += st_term_edge<VARIANT, i>(xb, nn, N);
-                }
-            };
-            st_static_for(harmonic, std::make_integer_sequence<int, hi - lo + 1>{});
-            emit(l);
-        } else if ((OUT & 3) != HS_OUT_REDUCED) {
-            emit(l);
-        } else {
-            tail = true;
-        }
-    };
-    st_static_for(level, std::make_integer_sequence<int, L - 1>{});
-    // With S unchanged over the skipped levels h_l = S c_l is monotone in l: testing the last level alone is enough.
-    if ((OUT & 3) == HS_OUT_REDUCED && tail) emit(L - 1);
-    if ((OUT & HS_OUT_REDUCED) && live && (OUT & HS_OUT_CAND)) {
-        hs_push(p.sink, b, n, e.m, e.a);
-    } else if ((OUT & HS_OUT_REDUCED) && live) {
-        hsptx::st_cs(p.vmax + (int64_t)b * N + n, e.m);
-        hsptx::st_cs(p.amax + (int64_t)b * N + n, (uint8_t)e.a);
-    }
-}
-
-struct st_sched {
-    gr_layout lay;
-    int64_t wave, slots;   // spectra per wave, workspace slots
-    int nchunks, n_split;
-};
-
-st_sched st_make_sched(const hs_plan *p, int64_t batch)
-{
-    st_sched s{};
-    const int N = (int)p->nbins;
-    s.lay = make_layout(N, p->Hmax, p->variant, 1);
-    s.nchunks = (N + kChunk - 1) / kChunk;
-    s.n_split = (int)(((int64_t)(N + 1) / 2 + kChunk - 1) / kChunk * kChunk);
-    int64_t wave = batch < 32768 ? batch : 32768;                       // gridDim.y
-    if (getenv("HS_ST_WAVE")) wave = atoi(getenv("HS_ST_WAVE"));
-    if (wave < 1) wave = 1;
-    if (wave > batch) wave = batch;
-    if (wave > 32768) wave = 32768;
-    s.wave = wave;
-    s.slots = wave;
-    return s;
-}
-
-template <int VARIANT, int HMAX, int OUT>
-int st_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
-{
-    const st_sched s = st_make_sched(p, batch);
-    gr_params prm{};
-    prm.x = buf.x;
-    prm.A = static_cast<float *>(ws);
-    prm.sums = buf.sums;
-    prm.vmax = buf.vmax;
-    prm.amax = buf.amax;
-    prm.sink = buf.sink;
-    prm.lay = s.lay;
-    prm.N = (int)p->nbins;
-    prm.B = (int)batch;
-    prm.groups = (int)s.slots;
-    prm.nchunks = s.nchunks;
-    prm.n_split = s.n_split;
-    auto kA = st_phaseA_kernel<VARIANT, HMAX, OUT>;
-    auto kB = st_phaseB_kernel<VARIANT, HMAX, OUT>;
-    const size_t smem = smem_bytes(VARIANT, HMAX) + (VARIANT == HS_MAX ? 0 : 0);
-    static bool configured = false;
-    if (!configured) {
-        HS_CUDA_OK(cudaFuncSetAttribute(kA, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
-    }
-    const int n_end = s.n_split < prm.N ? s.n_split : prm.N;
-    const unsigned tilesB = (unsigned)((n_end + kStThreads - 1) / kStThreads);
-    for (int64_t b0 = 0; b0 < batch; b0 += s.wave) {
-        const unsigned nb = (unsigned)(batch - b0 < s.wave ? batch - b0 : s.wave);
-        kA<<<dim3((unsigned)s.nchunks, nb), kThreads, smem, stream>>>(prm, (int)b0);
-        kB<<<dim3(tilesB, nb), kStThreads, 0, stream>>>(prm, (int)b0);
-    }
-    HS_CUDA_OK(cudaGetLastError());
-    return HS_OK;
-}
-
-template <int VARIANT, int HMAX>
-int st_by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
-{
-    switch (p->out_mode) {
-        case HS_OUT_FULL: return st_launch<VARIANT, HMAX, HS_OUT_FULL>(p, buf, batch, ws, stream);
-        case HS_OUT_REDUCED:
-            if (buf.sink.cand) return st_launch<VARIANT, HMAX, HS_OUT_REDUCED | HS_OUT_CAND>(p, buf, batch, ws, stream);
-            return st_launch<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, batch, ws, stream);
-        default: return st_launch<VARIANT, HMAX, HS_OUT_BOTH>(p, buf, batch, ws, stream);
-    }
-}
-
-template <int VARIANT>
-int st_by_hmax(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
-{
-    if (p->Hmax == 16) return st_by_out<VARIANT, 16>(p, buf, batch, ws, stream);
-    return st_by_out<VARIANT, 32>(p, buf, batch, ws, stream);
-}
-
 }  // namespace
 
 // One slot per group must fit the L2 budget: spectra of up to ~2^22 bins; Hmax = 1 has no phase A at all.
 bool hs_grouped_supported(const hs_plan *p)
 {
     if (p->variant != HS_MAX && p->variant != HS_FREQBIN) return false;
-    if (p->Hmax < 2) return false;
+    if (p->Hmax < 2 || p->nbins > ((int64_t)1 << 23)) return false;   // (the contract of HS_ALGO_GROUPED, include/hs.h)
     const gr_sched s = make_sched(p, p->batch);
     return (size_t)s.groups * (size_t)s.lay.slot_words * 4 <= 2 * kL2Budget;
 }
@@ -1088,31 +808,4 @@ int hs_grouped_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, vo
     if (!ws) HS_FAIL(HS_ERR_WORKSPACE);
     if (p->variant == HS_FREQBIN) return by_hmax<HS_FREQBIN>(p, buf, batch, ws, stream);
     return by_hmax<HS_MAX>(p, buf, batch, ws, stream);
-}
-
-// ---- streamed mode
-bool hs_streamed_supported(const hs_plan *p)
-{
-    if (p->variant != HS_MAX && p->variant != HS_FREQBIN) return false;
-    if (!st_hmax_ok(p->Hmax)) return false;
-    return p->nbins * 4 + 64 < ((int64_t)1 << 31);                     // word offsets inside a slot are 32-bit
-}
-
-size_t hs_streamed_workspace_bytes(const hs_plan *p, int64_t batch)
-{
-    const st_sched s = st_make_sched(p, batch);
-    return (size_t)s.slots * (size_t)s.lay.slot_words * 4 + 256;
-}
-
-int hs_streamed_launches(const hs_plan *p, int64_t batch)
-{
-    const st_sched s = st_make_sched(p, batch);
-    return (int)(2 * ((batch + s.wave - 1) / s.wave));
-}
-
-int hs_streamed_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
-{
-    if (!ws) HS_FAIL(HS_ERR_WORKSPACE);
-    if (p->variant == HS_FREQBIN) return st_by_hmax<HS_FREQBIN>(p, buf, batch, ws, stream);
-    return st_by_hmax<HS_MAX>(p, buf, batch, ws, stream);
 }

@@ -1,14 +1,15 @@
-// hs_interleaved.cu — eqs. 3 and 4 (CONVENTIONS.md C3, C4, C5) as a gather from a
-// spectrum-interleaved copy of a small group of spectra that lives in L2, run by ONE persistent kernel.
+// hs_interleaved.cu — eq. 3 (CONVENTIONS.md C3, C5) as a gather from a spectrum-interleaved copy of a
+// small group of spectra that lives in L2, run by ONE persistent kernel.
 //
-// Both variants read x(i n [+ j]) for i = 1..Hmax: a stride-i gather.  From the [batch][nbins] layout a warp of 32
-// consecutive n touches one 32-byte sector (and one 128-byte L1 line) per useful word for i >= 8, which is what bounds
-// the plain gather kernel (hs_greedy_gather.cu: one L1 wavefront per bin, 75-81 B/bin between L2 and the SMs).  Loop
-// inversion over the batch fixes it: G = 16 spectra are first copied into xT[k][g] (bin-major, the 16 spectra of a
-// group side by side: one 64-byte row per bin), and the gather runs with the lanes of a half-warp across the spectra
-// g, so every load instruction reads whole rows: full sectors whatever the stride, 4.06 (eq. 3) or 7.12 (eq. 4) words
-// per bin between L2 and the SMs.  A group's copy is 16 N floats (16 MiB at 2^18 bins) in a ring of R slots that stays
-// in L2: HBM sees x once (streamed, evict-first) and the outputs once (streaming stores).
+// Eq. 3 reads x(i n) for i = 1..Hmax: a stride-i gather.  From the [batch][nbins] layout a warp of 32 consecutive n
+// touches one 32-byte sector (and one 128-byte L1 line) per useful word for i >= 8, which is what bounds the plain
+// gather kernel (hs_greedy_gather.cu: 75 B/bin between L2 and the SMs).  Loop inversion over the batch fixes it: G = 16
+// spectra are first copied into xT[k][g] (bin-major, the 16 spectra of a group side by side: one 64-byte row per bin),
+// and the gather runs with four lanes across a row, so every load instruction reads whole rows: full sectors whatever
+// the stride, 4.06 words per bin between L2 and the SMs.  A group's copy is 16 N floats (16 MiB at 2^18 bins) in a
+// ring of R slots that stays in L2: HBM sees x once (streamed, evict-first) and the outputs once (streaming stores).
+// (Eq. 4 gains nothing from this layout: its two candidates sit at i n + j with a per-spectrum drift j, so neighbouring
+// spectra share a sector only while all j agree, and 16 spectra touch as many sectors as 16 bins do: DESIGN.md §7.)
 //
 // Work items, handed out in order from one global counter, step s = 0, 1, ..:
 //     T(s):   copy 512 bins x 16 spectra of group s into its ring slot; bins n >= N/2 have no harmonic but the first
@@ -25,14 +26,12 @@
 // ever wait for items handed out EARLIER, and an item is handed out to a CTA that is running, so the schedule cannot
 // deadlock and needs no co-residency.
 //
-// Gather thread = (spectrum g of the group, C = 8 consecutive bins): 8 independent chains per thread hide Greedy's
-// serial dependence j -> address -> load, and the outputs of a thread are two float4 and two 4-byte stores.  Range
-// handling is warp-uniform (a warp owns 16 consecutive bins): harmonic i is in range for every lane iff
-// i (n_hi + 1) <= N.
-#include <cstdlib>
-
+// Gather thread = (4 spectra of the group, C = 4 consecutive bins): one 16-byte load per bin and harmonic serves four
+// spectra, the outputs of a thread are four float4 and four 4-byte stores.  Range handling is warp-uniform (a warp owns
+// 32 consecutive bins): harmonic i is in range for every lane iff i (n_hi + 1) <= N.
 #include "hs_internal.cuh"
 #include "hs_ptx.cuh"
+#include "hs_sync.cuh"
 
 namespace {
 
@@ -59,7 +58,9 @@ struct il_params {
     float *sums;
     float *vmax;
     uint8_t *amax;
-    int *ctrl;          // [0] work counter, [1] error flag, [2..5] wait statistics, [16 + g] T items done, [16 + groups + g] G items done
+    int *ctrl;          // control block (hs_internal.cuh): [0] work counter, [1] error flag, [2..3] waits of T items for
+                        // their ring slot, [4..5] waits of G items for their copies; [16 + g] T items done, [16 + groups + g] G items done
+    unsigned spin_limit;
     int64_t slot_words;
     int N, B, groups, R, lag, order;
     int K;              // groups per step (order 1): short spectra need several groups for a step of a few rounds
@@ -75,30 +76,6 @@ __device__ __forceinline__ float4 ld_stream(const float4 *p)   // read-once inpu
     asm volatile("ld.global.cs.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
     return v;
 }
-__device__ __forceinline__ int ld_acquire(const int *p)
-{
-    int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-
-// thread 0 only: wait until *cnt >= target (bounded: a bug must not hang the GPU; the error flag makes it visible)
-__device__ __forceinline__ void wait_count(const int *cnt, int target, int *err, int *stat)
-{
-    unsigned spins = 0;
-    while (ld_acquire(cnt) < target) {
-        __nanosleep(64);
-        if (++spins > (1u << 23)) {
-            atomicExch(err, 1);
-            break;
-        }
-    }
-    if (spins) {
-        atomicAdd(stat, 1);
-        atomicAdd(stat + 1, (int)(spins > 0x7fffu ? 0x7fffu : spins));
-    }
-}
-
 // ------------------------------------------------------------------------------------------------ T item
 // xT[k][g] = x[b0 + g][k] for g < nb, 0 for nb <= g < G, k in [k0, k0 + 512) below N; outputs of the bins >= n_split.
 template <int L, int OUT>
@@ -334,7 +311,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
 {
     __shared__ __align__(16) float tile[G * kTStride];
     __shared__ int s_item;
-    int *queue = p.ctrl, *err = p.ctrl + 1;
+    int *queue = p.ctrl + HS_CTRL_QUEUE;
     int *doneT = p.ctrl + 16, *doneG = p.ctrl + 16 + p.groups;
     const int per = p.nT + p.nG, per_step = p.K * per;
     const int total = ((p.groups + p.K - 1) / p.K + p.lag) * per_step;
@@ -366,7 +343,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
             if (s < p.groups) {
                 float *xT = p.xT + (int64_t)(s % p.R) * p.slot_words;
                 if (threadIdx.x == 0 && s >= p.R && p.nG > 0 && lastG < s - p.R) {
-                    wait_count(doneG + (s - p.R), p.nG, err, p.ctrl + 2);
+                    hssync::wait_count(doneG + (s - p.R), p.nG, p.ctrl, p.ctrl + 2, p.spin_limit);
                     lastG = s - p.R;
                 }
                 __syncthreads();
@@ -381,7 +358,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
             const int grp = s;
             const float *xT = p.xT + (int64_t)(grp % p.R) * p.slot_words;
             if (threadIdx.x == 0 && lastT < grp) {
-                wait_count(doneT + grp, p.nT, err, p.ctrl + 4);
+                hssync::wait_count(doneT + grp, p.nT, p.ctrl, p.ctrl + 4, p.spin_limit);
                 lastT = grp;
             }
             __syncthreads();
@@ -418,8 +395,10 @@ il_sched make_sched(const hs_plan *p, int64_t batch)
     s.groups = (int)((batch + G - 1) / G);
     int ring = kMaxRing;
     s.lag = kLagDefault;
-    if (getenv("HS_IL_RING")) ring = atoi(getenv("HS_IL_RING"));
-    if (getenv("HS_IL_LAG")) s.lag = atoi(getenv("HS_IL_LAG"));
+    ring = hs_knob("HS_IL_RING", ring);
+    s.lag = hs_knob("HS_IL_LAG", s.lag);
+    if (s.lag < 1) s.lag = 1;
+    if (ring < s.lag + 2) ring = s.lag + 2;                            // a slot is rewritten only after its gather was handed out
     s.nT = (N + kTBins - 1) / kTBins;
     // bins n >= N/2 have S_H(n) = x(n): the T items emit them.  The split is a multiple of the T tile.
     const int half = (N + 1) / 2;
@@ -436,8 +415,8 @@ il_sched make_sched(const hs_plan *p, int64_t batch)
     // one group of 2^18-bin spectra is that long, shorter spectra take several (the ring stays 48 MiB)
     const int per = s.nT + s.nG;
     int K = (int)((2.6 * 2 * p->sm_count + per / 2) / per);
-    if (getenv("HS_IL_K")) K = atoi(getenv("HS_IL_K"));
-    if (K < 1 || getenv("HS_IL_ORDER")) K = 1;
+    K = hs_knob("HS_IL_K", K);
+    if (K < 1 || hs_knob("HS_IL_ORDER", 1) != 1) K = 1;
     s.K = K;
     ring *= K;
     s.R = s.groups < ring ? s.groups : ring;
@@ -465,18 +444,16 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.R = s.R;
     prm.lag = s.lag;
     prm.K = s.K;
-    prm.order = getenv("HS_IL_ORDER") ? atoi(getenv("HS_IL_ORDER")) : 1;
+    prm.order = hs_knob("HS_IL_ORDER", 1);
+    prm.spin_limit = hs_spin_limit();
     prm.nT = s.nT;
     prm.nG = s.nG;
     prm.nHeavy = s.nHeavy;
     prm.n_split = s.n_split;
     auto kern = il_persistent_kernel<L, OUT>;
-    static int ctas_per_sm = 0;
-    if (ctas_per_sm == 0) {
-        int occ = 0;
-        HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, 0));
-        ctas_per_sm = occ > 0 ? occ : 1;
-    }
+    int occ = 0;                                                        // (per device: asked on every launch)
+    HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, 0));
+    const int ctas_per_sm = occ > 0 ? occ : 1;
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(s.groups), stream));
     const int64_t total = (int64_t)((s.groups + s.K - 1) / s.K + s.lag) * s.K * (s.nT + s.nG);
     const int64_t slots = (int64_t)p->sm_count * ctas_per_sm;

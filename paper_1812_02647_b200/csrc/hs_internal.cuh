@@ -4,6 +4,9 @@
 #include <cuda_runtime.h>
 #include <stddef.h>
 #include <stdint.h>
+#ifdef HS_TUNING
+#include <cstdlib>
+#endif
 
 #include "../../include/hs.h"
 
@@ -11,13 +14,39 @@
 #define HS_OUT_CAND 8   // internal OUT template bit: reduced output goes to the candidate sink (hs_execute_candidates)
 #define HS_HOST_LANES 3
 
+// Control block at the start of every workspace that a persistent kernel synchronises through (zeroed by a memset
+// node before each launch): word 0 = work counter, word 1 = error flag (a bounded wait gave up, hs_plan_device_status),
+// words 2.. = wait statistics of the kernel family.
+#define HS_CTRL_QUEUE 0
+#define HS_CTRL_ERROR 1
+#define HS_CTRL_STATS 2
+#define HS_SPIN_LIMIT_DEFAULT (1u << 23)
+
+// Tuning knobs are compiled out of the product: only a -DHS_TUNING build (the builder's sweeps and the forced-timeout
+// test, libhs_tuning.so) reads the environment.
+inline int hs_knob(const char *name, int dflt)
+{
+#ifdef HS_TUNING
+    const char *v = getenv(name);
+    return v ? atoi(v) : dflt;
+#else
+    (void)name;
+    return dflt;
+#endif
+}
+inline unsigned hs_spin_limit() { return (unsigned)hs_knob("HS_SPIN_LIMIT", (int)HS_SPIN_LIMIT_DEFAULT); }
+
 struct hs_plan {
     int64_t nbins, batch;
     int Hmax, L, variant, out_mode;
     int algo_req;  // what the caller asked for (enum hs_algo)
     int algo;      // resolved family, never AUTO
+    int device;    // ordinal of the device the plan was created on (checked at execute)
     int sm_count;
     size_t smem_optin;  // max dynamic shared memory per block
+    // control blocks (device) the last execute launched with, for hs_plan_device_status; written by hs_execute*
+    mutable const void *last_ctrl[3];
+    mutable int n_last_ctrl;
     // workspace for the resolved algorithm (device, caller-owned)
     void *ws;
     size_t ws_bytes;
@@ -90,10 +119,7 @@ int hs_grouped_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, vo
 int hs_grouped_launches(const hs_plan *p, int64_t batch);
 size_t hs_grouped_workspace_bytes(const hs_plan *p, int64_t batch);
 bool hs_grouped_supported(const hs_plan *p);
-int hs_streamed_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
-int hs_streamed_launches(const hs_plan *p, int64_t batch);
-size_t hs_streamed_workspace_bytes(const hs_plan *p, int64_t batch);
-bool hs_streamed_supported(const hs_plan *p);
+bool hs_tiled_has_ctrl(const hs_plan *p);   // the resolved kernel starts its workspace with a control block
 
 // ---- device-side epilogue ---------------------------------------------------------------------------------------
 // c_H = fp32(1/sqrt(H)) for H = 1,2,4,8,16,32 (CONVENTIONS.md C7; "1/sqrt(H)").

@@ -292,12 +292,9 @@ int hs_standard_rb_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch
     prm.counter = static_cast<int *>(ws);
     prm.sink = buf.sink;
     const size_t smem = (size_t)(kSlots * kSlot) * sizeof(float);
-    static bool configured = false;
-    if (!configured) {
-        HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
-    }
+    // (function attributes are per device: set on every launch rather than once per process)
+    if (buf.sink.cand) HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    else HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t slots = (int64_t)p->sm_count * kCtasPerSm;
     const unsigned grid = (unsigned)(prm.tiles < slots ? prm.tiles : slots);
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, 256, stream));

@@ -100,12 +100,9 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
     const int N = (int)p->nbins;
     const int tiles = (N + T - 1) / T;
     const size_t smem = (size_t)(T * (HMAX + 1) / 2 + 8 * HMAX + 8) * sizeof(float);
-    static bool configured = false;
     auto kern = hs_std_tiled_kernel<HMAX, OUT, WARPS, STEPS>;
-    if (!configured) {
-        HS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured = true;
-    }
+    // (function attributes are per device: set on every launch rather than once per process)
+    HS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t max_spectra = ((int64_t)1 << 30) / tiles;
     for (int64_t b0 = 0; b0 < batch; b0 += max_spectra) {
         const int64_t nb = (batch - b0 < max_spectra) ? batch - b0 : max_spectra;

@@ -1,28 +1,22 @@
-// hs_twophase.cu — eqs. 2 and 3 (CONVENTIONS.md C2, C3, C5) in two phases through a small ring of
-// workspace slots that stays resident in the 126 MB L2, run by ONE persistent kernel.
+// hs_twophase.cu — eqs. 2 and 3 (CONVENTIONS.md C2, C3, C5) in two phases as two plain kernels per
+// group of spectra, the per-harmonic arrays going through HBM: the fallback for spectra whose arrays do not fit the
+// L2-resident schemes (hs_ring_max.cu / hs_grouped.cu / hs_interleaved.cu), valid for any spectrum length.
 //
 // Both variants have the form S_H(n) = sum_{i<=H} A_i(n) with a per-harmonic array that depends on x only:
 //     freq-bin  A_i(n) = x~(i n)                      the stride-i decimation of the spectrum
 //     Max       A_i(n) = max x~[i n .. i n + i - 1]   the maximum of the aligned block of size i
 // A_i has ceil(N/i) non-zero entries, sum_{i=2..32} N/i = 3.06 N words in all.  Gathering x(i n) per output touches one
 // 32-byte sector per word for i >= 8 and, for Max, re-reads the spectrum once per harmonic; instead
-//   phase 1 (item = one 4096-word input chunk) reads the chunk ONCE, coalesced, into shared memory and writes every
+//   phase 1 (one CTA per 4096-word input chunk) reads the chunk ONCE, coalesced, into shared memory and writes every
 //           A_i segment it owns;
-//   phase 2 (item = 4096 outputs) reads x and the A_i with unit stride (float4), accumulates the levels, normalises and
-//           emits the outputs.
-// Work items are handed out in order from one global counter: [phase 1 of spectrum b][phase 2 of spectrum b - D] for
-// b = 0, 1, ...  A phase-2 item waits (acquire load on a per-spectrum counter) until all chunks of its spectrum are
-// written; a phase-1 item waits until phase 2 of the spectrum that last used its ring slot (b - R) is finished.  Items
-// only ever wait for items handed out EARLIER, so the schedule cannot deadlock, and with D of a few spectra the waits
-// are never actually exercised: the lag hides them.  The ring has R = 2 D slots, a few tens of MB: the A traffic
-// (3.06 N words written, 3.06 N read per spectrum) stays in L2 and HBM sees x once and the outputs once.
+//   phase 2 (one CTA per 4096 outputs) reads x and the A_i with unit stride (float4), accumulates the levels,
+//           normalises and emits the outputs.
+// Stream order is the only synchronisation.  HBM traffic: x twice, the arrays written and read once, the outputs once.
 //
 // Max, phase 1: for odd j the blocks of size j are reduced by one thread each (lane stride j words: conflict-free);
 // the blocks of size 2j, 4j, .. <= Hmax are unions of aligned pairs, so they come from a shuffle-xor pyramid over
 // neighbouring lanes (M_2j(n) = max(M_j(2n), M_j(2n+1))).  A chunk owns the super-blocks (size j*K_j, K_j the largest
 // power of two with j*K_j <= Hmax) that START inside it, and reads a 32-word halo for those that run past its end.
-#include <cstdlib>
-
 #include "hs_internal.cuh"
 #include "hs_ptx.cuh"
 
@@ -62,15 +56,12 @@ struct tp_params {
     float *vmax;
     uint8_t *amax;
     hs_cand_sink sink;
-    int *ctrl;       // [0] work counter, [1] error flag, [2..5] wait statistics, [16 + b] phase-1 chunks done, [16 + B + b] phase-2 tiles done
     tp_layout lay;
     int N;
     int B;
     int nchunks;     // phase-1 items per spectrum (0 when Hmax == 1)
     int ntiles;      // phase-2 items per spectrum
-    int D;           // phase 2 lags phase 1 by D spectra
-    int R;           // ring slots
-    int discard;     // drop consumed A lines from L2 without write-back
+    int R;           // workspace slots = spectra per kernel pair
 };
 
 constexpr int chain_len(int j, int hmax)  // K_j: largest power of two with j*K <= hmax
@@ -78,34 +69,6 @@ constexpr int chain_len(int j, int hmax)  // K_j: largest power of two with j*K 
     int k = 1;
     while (j * k * 2 <= hmax) k *= 2;
     return k;
-}
-
-__device__ __forceinline__ int ld_acquire(const int *p)
-{
-    int v;
-    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void red_release_add(int *p, int v)
-{
-    asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-
-// thread 0 only: wait until *cnt >= target (bounded: a bug must not hang the GPU; the error flag makes it visible)
-__device__ __forceinline__ void wait_count(const int *cnt, int target, int *err, int *stat)
-{
-    unsigned spins = 0;
-    while (ld_acquire(cnt) < target) {
-        __nanosleep(64);
-        if (++spins > (1u << 22) || ld_acquire(err) != 0) {
-            atomicExch(err, 1);
-            break;
-        }
-    }
-    if (spins) {                      // statistics for tuning the lag: [stat] waits that had to spin, [stat+1] spins
-        atomicAdd(stat, 1);
-        atomicAdd(stat + 1, (int)spins);
-    }
 }
 
 // ---------------------------------------------------------------------------------------------- phase 1
@@ -255,10 +218,6 @@ __device__ __forceinline__ void phase2_round(const tp_params &p, const float *__
                     S.y += v.y;
                     S.z += v.z;
                     S.w += v.w;
-                    // This 128-byte line of A_i is read by exactly these 8 lanes and never again: drop it from L2 so
-                    // that the dead data is not written back to HBM.  The test on v.x makes the discard wait for the load.
-                    if (p.discard && (threadIdx.x & 7) == 0 && v.x == v.x)
-                        asm volatile("discard.global.L2 [%0], 128;" ::"l"(An + p.lay.off[i]) : "memory");
                 }
             } else {
 #pragma unroll
@@ -298,27 +257,12 @@ __device__ __forceinline__ void phase2_round(const tp_params &p, const float *__
     }
 }
 
-// ---------------------------------------------------------------------------------------------- persistent kernel
+// ---------------------------------------------------------------------------------------------- kernels
 struct tp_item {
     int kind;   // 0 = nothing to do, 1 = phase 1, 2 = phase 2
     int b;      // spectrum
     int idx;    // chunk (phase 1) or tile (phase 2)
 };
-
-__device__ __forceinline__ tp_item decode_item(const tp_params &p, int item, int64_t total)
-{
-    tp_item it{0, 0, 0};
-    if (item >= total) return it;
-    const int per_round = p.nchunks + p.ntiles;
-    const int r = item / per_round, rem = item - r * per_round;
-    if (rem < p.nchunks) {
-        if (r < p.B) it = tp_item{1, r, rem};
-    } else {
-        const int b = r - p.D;
-        if (b >= 0 && b < p.B) it = tp_item{2, b, rem - p.nchunks};
-    }
-    return it;
-}
 
 // Issue the global loads of an item's input (x only: it never depends on another item) into registers.
 __device__ __forceinline__ void preload(const tp_params &p, const tp_item &it, tp_pre &pre)
@@ -339,91 +283,7 @@ __device__ __forceinline__ void preload(const tp_params &p, const tp_item &it, t
     }
 }
 
-template <int VARIANT, int HMAX, int OUT>
-__global__ void __launch_bounds__(kThreads, kMinCtasPerSm)
-tp_persistent_kernel(const __grid_constant__ tp_params p)
-{
-    static_assert(kChunk == kTile2, "preload() addresses both phases the same way");
-    constexpr int L = HMAX == 1 ? 1 : HMAX == 2 ? 2 : HMAX == 4 ? 3 : HMAX == 8 ? 4 : HMAX == 16 ? 5 : 6;
-    __shared__ __align__(16) float sm[kChunk + kHalo + 16];        // + zero pad read by the table builds
-    __shared__ int2 s_bounds[33];
-    __shared__ int s_item[2];
-    int *queue = p.ctrl, *err = p.ctrl + 1;
-    int *cnt1 = p.ctrl + 16, *cnt2 = p.ctrl + 16 + p.B;
-    const int64_t total = (int64_t)(p.B + p.D) * (p.nchunks + p.ntiles);
-    const int N = p.N;
-
-    if (threadIdx.x < 16) sm[kChunk + kHalo + threadIdx.x] = 0.0f;
-    if (threadIdx.x == 0) {
-        s_item[0] = atomicAdd(queue, 1);
-        s_item[1] = atomicAdd(queue, 1);
-    }
-    __syncthreads();
-    int item = s_item[0], next = s_item[1];
-    __syncthreads();
-    tp_item cur = decode_item(p, item, total);
-    tp_pre pre;
-    preload(p, cur, pre);
-    int flip = 0;
-    while (item < total) {
-        int after = 0;
-        if (threadIdx.x == 0) after = atomicAdd(queue, 1);           // consumed only at the end of this iteration
-        const tp_item nxt = decode_item(p, next, total);
-        if (cur.kind == 1) {                                         // ---- phase 1: chunk cur.idx of spectrum cur.b
-            const int b = cur.b, k0 = cur.idx * kChunk;
-#pragma unroll
-            for (int q = 0; q < kChunk / (4 * kThreads); q++)
-                reinterpret_cast<float4 *>(sm)[q * kThreads + threadIdx.x] = pre.v[q];
-            if (threadIdx.x < kHalo / 4) reinterpret_cast<float4 *>(sm)[kChunk / 4 + threadIdx.x] = pre.halo;
-            if (threadIdx.x >= 2 && threadIdx.x <= HMAX) {
-                const int i = threadIdx.x;
-                s_bounds[i] = make_int2((k0 + i - 1) / i, min((k0 + kChunk + i - 1) / i, p.lay.len[i]));
-            }
-            preload(p, nxt, pre);                                    // in flight while this item computes
-            // the ring slot is free once phase 2 of the spectrum that used it last (b - R) has finished
-            if (threadIdx.x == 0 && b >= p.R) wait_count(cnt2 + (b - p.R), p.ntiles, err, p.ctrl + 2);
-            __syncthreads();
-            float *Ab = p.A + (int64_t)(b % p.R) * p.lay.slot_words;
-            if (VARIANT == HS_FREQBIN) decimate_chunk<HMAX>(p, sm - k0, s_bounds, Ab);
-            else blockmax_chunk<HMAX>(p, sm, s_bounds, Ab, k0);
-            if (threadIdx.x == 0) s_item[flip] = after;
-            __syncthreads();                                         // all stores of the CTA are ordered before ...
-            if (threadIdx.x == 0) red_release_add(cnt1 + b, 1);      // ... thread 0's release (cumulative, gpu scope)
-        } else if (cur.kind == 2) {                                  // ---- phase 2: 4096 outputs of spectrum cur.b
-            const int b = cur.b;
-            const int64_t row = (int64_t)b * N;
-            const int n0 = cur.idx * kTile2 + 4 * threadIdx.x;
-            float4 S[kRounds2];
-#pragma unroll
-            for (int q = 0; q < kRounds2; q++) S[q] = pre.v[q];
-            preload(p, nxt, pre);
-            if (threadIdx.x == 0 && p.nchunks > 0) wait_count(cnt1 + b, p.nchunks, err, p.ctrl + 4);
-            __syncthreads();
-            const float *Ab = p.A + (int64_t)(b % p.R) * p.lay.slot_words;
-#pragma unroll
-            for (int q = 0; q < kRounds2; q++) {
-                const int n = n0 + q * (4 * kThreads);
-                if (n < N) phase2_round<L, OUT>(p, Ab, row, n, S[q]);
-            }
-            if (threadIdx.x == 0) s_item[flip] = after;
-            __syncthreads();
-            if (threadIdx.x == 0) red_release_add(cnt2 + b, 1);
-        } else {
-            preload(p, nxt, pre);
-            if (threadIdx.x == 0) s_item[flip] = after;
-            __syncthreads();
-        }
-        item = next;
-        cur = nxt;
-        next = s_item[flip];
-        flip ^= 1;
-    }
-}
-
-// ---------------------------------------------------------------------------------------------- plain two-launch path
-// The same phase bodies as two ordinary kernels over a group of spectra (one CTA per item, the hardware scheduler
-// instead of the work counter, stream order instead of the dependency counters).  Each kernel has its own register
-// budget, so more CTAs fit per SM than in the fused persistent kernel.
+// The phase bodies as two ordinary kernels over a group of spectra (one CTA per item).
 template <int VARIANT, int HMAX>
 __global__ void __launch_bounds__(kThreads, 6)
 tp_phase1_kernel(const __grid_constant__ tp_params p, int b0)
@@ -470,16 +330,8 @@ tp_phase2_kernel(const __grid_constant__ tp_params p, int b0)
     }
 }
 
-// tuning knobs for experiments (environment, read when the schedule is built); defaults are the tuned values
-int tune_int(const char *name, int dflt)
-{
-    const char *v = getenv(name);
-    return v && *v ? atoi(v) : dflt;
-}
-
 struct tp_sched {
-    int nchunks, ntiles, D, R, grid;
-    bool plain;
+    int nchunks, ntiles, R;
     tp_layout lay;
 };
 
@@ -490,40 +342,14 @@ tp_sched make_sched(const hs_plan *p, int64_t batch)
     s.lay = make_layout(N, p->Hmax);
     s.nchunks = p->Hmax > 1 ? (N + kChunk - 1) / kChunk : 0;
     s.ntiles = (N + kTile2 - 1) / kTile2;
-    s.grid = p->sm_count * tune_int("HS_TP_CTAS", kMinCtasPerSm);
-    const int per_round = s.nchunks + s.ntiles;
-    // lag: enough rounds that the CTAs in flight never reach a phase-2 item before its phase-1 items have finished
-    (void)per_round;
-    // Items are claimed in order but finish out of order: a CTA holds up to three claimed items (running, preloaded,
-    // prefetched index), and a phase-2 item that has to spin delays the phase-1 items queued behind it in the same CTA,
-    // which in turn makes later phase-2 items spin (a convoy).  Measured on B200 (profiles/r01_twophase_lag.md): with
-    // 4 CTAs/SM the spinning only vanishes once phase 2 lags by about six times the items in flight, and the ring
-    // needs as much slack again.  That is ~0.8 GB of workspace whatever the spectrum length; it no longer fits L2.
-    const int in_flight = s.nchunks > 0 ? (6 * s.grid + s.nchunks - 1) / s.nchunks : 0;
-    int D = tune_int("HS_TP_LAG", in_flight + 1);
-    if (D > batch) D = (int)batch;
-    if (D < 1) D = 1;
-    int R = tune_int("HS_TP_RING", 4 * D);
-    if (R > batch) R = (int)batch;
-    if (R < D) R = D;          // (R >= D keeps slot b-R's phase 2 strictly before phase 1 of b in the item order)
-    s.D = D;
-    s.R = R < 1 ? 1 : R;
-    s.plain = tune_int("HS_TP_MODE", 1) == 1;
-    if (s.plain) {
-        // plain two-launch mode: groups of up to 512 spectra (1.6 GB of A arrays at 2^18 bins); bigger groups mean
-        // fewer, longer kernels (B200: 256 -> 9.8 ms, 512 -> 9.2 ms, 1024 -> 8.6 ms for eq. 2 on 4096 x 2^18)
-        int64_t G = tune_int("HS_TP_RING", 0);
-        if (G <= 0) {
-            G = s.lay.slot_words > 0 ? ((int64_t)1600 << 20) / (s.lay.slot_words * 4) : batch;
-            if (G > 65535) G = 65535;
-        }
-        if (G > batch) G = batch;
-        s.R = G < 1 ? 1 : (int)G;
-    }
+    // groups of spectra whose arrays take up to 1.6 GB: bigger groups mean fewer, longer kernels
+    // (B200, eq. 2 on 4096 x 2^18: 256 spectra per group 9.8 ms, 512 9.2 ms, 1024 8.6 ms)
+    int64_t G = s.lay.slot_words > 0 ? ((int64_t)1600 << 20) / (s.lay.slot_words * 4) : batch;
+    if (G > 65535) G = 65535;                                          // gridDim.y
+    if (G > batch) G = batch;
+    s.R = G < 1 ? 1 : (int)G;
     return s;
 }
-
-size_t ctrl_bytes(int64_t batch) { return (size_t)((16 + 2 * batch) * sizeof(int) + 255) / 256 * 256; }
 
 template <int VARIANT, int HMAX, int OUT>
 int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
@@ -531,8 +357,7 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     const tp_sched s = make_sched(p, batch);
     tp_params prm{};
     prm.x = buf.x;
-    prm.ctrl = static_cast<int *>(ws);
-    prm.A = reinterpret_cast<float *>(static_cast<char *>(ws) + ctrl_bytes(batch));
+    prm.A = static_cast<float *>(ws);
     prm.sums = buf.sums;
     prm.vmax = buf.vmax;
     prm.amax = buf.amax;
@@ -542,28 +367,18 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.B = (int)batch;
     prm.nchunks = s.nchunks;
     prm.ntiles = s.ntiles;
-    prm.D = s.D;
     prm.R = s.R;
-    prm.discard = tune_int("HS_TP_DISCARD", 0);
-    if (s.plain) {
-        // plain path: groups of R spectra, phase 1 then phase 2 in stream order
-        constexpr int L = HMAX == 1 ? 1 : HMAX == 2 ? 2 : HMAX == 4 ? 3 : HMAX == 8 ? 4 : HMAX == 16 ? 5 : 6;
-        for (int64_t b0 = 0; b0 < batch; b0 += s.R) {
-            const int nb = (int)((batch - b0 < s.R) ? batch - b0 : s.R);
-            if (s.nchunks > 0) {
-                tp_phase1_kernel<VARIANT, HMAX><<<dim3((unsigned)s.nchunks, (unsigned)nb), kThreads, 0, stream>>>(prm, (int)b0);
-                HS_CUDA_OK(cudaGetLastError());
-            }
-            tp_phase2_kernel<L, OUT><<<dim3((unsigned)s.ntiles, (unsigned)nb), kThreads, 0, stream>>>(prm, (int)b0);
+    // groups of R spectra, phase 1 then phase 2 in stream order
+    constexpr int L = HMAX == 1 ? 1 : HMAX == 2 ? 2 : HMAX == 4 ? 3 : HMAX == 8 ? 4 : HMAX == 16 ? 5 : 6;
+    for (int64_t b0 = 0; b0 < batch; b0 += s.R) {
+        const int nb = (int)((batch - b0 < s.R) ? batch - b0 : s.R);
+        if (s.nchunks > 0) {
+            tp_phase1_kernel<VARIANT, HMAX><<<dim3((unsigned)s.nchunks, (unsigned)nb), kThreads, 0, stream>>>(prm, (int)b0);
             HS_CUDA_OK(cudaGetLastError());
         }
-        return HS_OK;
+        tp_phase2_kernel<L, OUT><<<dim3((unsigned)s.ntiles, (unsigned)nb), kThreads, 0, stream>>>(prm, (int)b0);
+        HS_CUDA_OK(cudaGetLastError());
     }
-    HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(batch), stream));
-    const int64_t total = (int64_t)(batch + s.D) * (s.nchunks + s.ntiles);
-    const unsigned grid = (unsigned)(total < s.grid ? total : s.grid);
-    tp_persistent_kernel<VARIANT, HMAX, OUT><<<grid, kThreads, 0, stream>>>(prm);
-    HS_CUDA_OK(cudaGetLastError());
     return HS_OK;
 }
 
@@ -596,22 +411,20 @@ int by_hmax(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cu
 
 size_t hs_twophase_workspace_bytes(const hs_plan *p, int64_t batch)
 {
-    // The work/dependency counters need batch <= 2^30 spectra and fewer than 2^31 items.
     const tp_sched s = make_sched(p, batch);
-    return ctrl_bytes(batch) + (size_t)s.R * (size_t)s.lay.slot_words * 4 + 256;
+    return (size_t)s.R * (size_t)s.lay.slot_words * 4 + 256;
 }
 
 int hs_twophase_launches(const hs_plan *p, int64_t batch)
 {
     const tp_sched s = make_sched(p, batch);
-    if (!s.plain) return 2;  // one memset node + one persistent kernel
     return (int)((batch + s.R - 1) / s.R) * (s.nchunks > 0 ? 2 : 1);
 }
 
 bool hs_twophase_supported(const hs_plan *p, int64_t batch)
 {
-    const tp_sched s = make_sched(p, batch);
-    return (batch + s.D) * (int64_t)(s.nchunks + s.ntiles) < ((int64_t)1 << 31) - (int64_t)s.grid * 4;
+    (void)batch;
+    return p->variant == HS_MAX || p->variant == HS_FREQBIN;
 }
 
 int hs_twophase_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
