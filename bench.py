@@ -321,6 +321,10 @@ def main():
     peak, peak_src = measured_peak()
     bpb = BYTES_PER_BIN[out_mode]
     per_variant = {}
+    default_kernels = {"standard": "rb_kernel", "max": "gr_kernel", "freqbin": "il_persistent_kernel",
+                       "greedy": "hs_greedy_gather_kernel"}
+    WAIT_WORDS = {"gr_kernel": "[group-barrier waits that had to spin, polls, -, -]",
+                  "il_persistent_kernel": "[times a CTA found neither of its tickets runnable, polls of those, -, -]"}
     for v in variants:
         gbs = bpb * batch * nbins / (per_variant_ms[v] * 1e-3) / 1e9
         per_variant[v] = {"ms": per_variant_ms[v], "best_ms": per_variant_best[v],
@@ -328,15 +332,14 @@ def main():
                           "frac_of_measured_peak": gbs / peak, "frac_of_nominal_8TBps": gbs / 8000.0,
                           "algo": algo_names[plans[v].algo], "launches": plans[v].launches()}
         ws = plans[v]._ws
-        if ws is not None and ws.numel() >= 64 and v in ("max", "freqbin"):
-            # two-phase kernel's dependency-wait statistics (workspace words 2..5, see hs_twophase.cu)
+        if ws is not None and ws.numel() >= 64 and v != "standard":
+            # wait statistics of the persistent kernels' control block (hs_internal.cuh: words 2.. of the workspace)
             c = ws[:64].view(torch.int32).cpu().tolist()
-            per_variant[v]["waits"] = {"ring_waits": c[2], "ring_spins": c[3], "phase2_waits": c[4], "phase2_spins": c[5],
+            per_variant[v]["waits"] = {"kernel": default_kernels.get(v), "error_flag": c[1], "words_2_to_5": c[2:6],
+                                       "meaning": WAIT_WORDS.get(default_kernels.get(v), "?"),
                                        "workspace_MiB": round(plans[v].workspace_bytes() / 2**20)}
     dominant = max(variants, key=lambda v: per_variant_ms[v])
     dom_algo = per_variant[dominant]["algo"]
-    default_kernels = {"standard": "rb_kernel", "max": "gr_kernel", "freqbin": "il_persistent_kernel",
-                       "greedy": "hs_greedy_gather_kernel"}
     kname = default_kernels[dominant] if (args.algo == "auto" and args.workload == "config2") else dom_algo
     roofline = {"bound": "hbm", "kernel": f"{kname} ({dominant}, eq. {1 + VARIANTS.index(dominant) if dominant in VARIANTS else 0})", "achieved": per_variant[dominant]["eff_GBps"],
                 "peak": peak, "unit": "GB/s", "frac": per_variant[dominant]["eff_GBps"] / peak,

@@ -2,33 +2,35 @@
 // small group of spectra that lives in L2, run by ONE persistent kernel.
 //
 // Eq. 3 reads x(i n) for i = 1..Hmax: a stride-i gather.  From the [batch][nbins] layout a warp of 32 consecutive n
-// touches one 32-byte sector (and one 128-byte L1 line) per useful word for i >= 8, which is what bounds the plain
-// gather kernel (hs_greedy_gather.cu: 75 B/bin between L2 and the SMs).  Loop inversion over the batch fixes it: G = 16
-// spectra are first copied into xT[k][g] (bin-major, the 16 spectra of a group side by side: one 64-byte row per bin),
-// and the gather runs with four lanes across a row, so every load instruction reads whole rows: full sectors whatever
-// the stride, 4.06 words per bin between L2 and the SMs.  A group's copy is 16 N floats (16 MiB at 2^18 bins) in a
-// ring of R slots that stays in L2: HBM sees x once (streamed, evict-first) and the outputs once (streaming stores).
-// (Eq. 4 gains nothing from this layout: its two candidates sit at i n + j with a per-spectrum drift j, so neighbouring
-// spectra share a sector only while all j agree, and 16 spectra touch as many sectors as 16 bins do: DESIGN.md §7.)
+// touches one 128-byte L1 line (and one 32-byte sector) per lane for large i, and the L1 of an SM looks up about one
+// line per clock (profiles/r02_microbench_b200.txt): that, not HBM, bounds the plain gather (hs_greedy_gather.cu).
+// Loop inversion over the batch fixes it: G = 16 spectra are first copied into a ring slot as xT[k][g] (bin-major, the
+// 16 spectra of a group side by side: one 64-byte row per bin), and the gather runs with four lanes across a row
+// (float4 = 4 spectra each): whole sectors whatever the stride, 4.06 words per bin between L2 and the SMs.  A group's
+// copy is 16 N floats (16 MiB at 2^18 bins) in a ring of R slots that stays in L2: HBM sees x once (streamed,
+// evict-first) and the outputs once (streaming stores).
+// (Eq. 4 was tried on this layout in round 2, with max(x(k), x(k+1)) and the comparison bit packed into one word so
+// that a harmonic costs ONE load: parity green, but 10.9 ms against the plain gather's 5.3 ms.  Greedy's 31 dependent
+// loads per bin make a group's gather phase ~31 L2 latencies long whatever the item size, and a ring that covers
+// throughput x that latency (Little's law: 1.4 TB/s x 50 us = 70 MB) does not fit the ~30 MB of L2 that stay dirty:
+// DESIGN.md section 7.)
 //
-// Work items, handed out in order from one global counter, step s = 0, 1, ..:
-//     T(s):   copy 512 bins x 16 spectra of group s into its ring slot; bins n >= N/2 have no harmonic but the first
-//             in range (S_H(n) = x(n) for every H), so their outputs are emitted right here, in the natural layout;
-//     G(s-1): 256 (bins below N/8) or 768 bins x 16 spectra of the gather for group s-1 (bins below N/2 only), low
-//             (= long) bins first;
-// Within a step all T items come first, then all G items.  A G item waits (acquire load on a per-group counter) until all
-// T items of its group are done: those were handed out in the first half of the previous step.  A T item waits until the
-// gather of the group that used its ring slot last (g - R, R = 3) is done: handed out in the second half of step s - 2.
-// Every dependence therefore points at least a full step (~2.7 rounds of the resident CTAs) back and nothing waits, with a
-// ring of only 3 x 16 MiB = 48 MiB: proportional interleaving of the T and G items needed R = 4, lag 2 for that, and the
-// larger ring was written back to HBM almost entirely (4.30 -> 3.85 ms, profiles/r01_experiments.md).  CTAs drift apart
-// within a step, so the HBM-bound copies and the L2-bound gathers still overlap on the machine as a whole.  Items only
-// ever wait for items handed out EARLIER, and an item is handed out to a CTA that is running, so the schedule cannot
-// deadlock and needs no co-residency.
+// Work items and scheduling.  Two kinds of items, each kind handed out in order from its own global counter:
+//     T item: copy 512 bins x 16 spectra of a group into its ring slot; bins n >= N/2 have no harmonic but the first in
+//             range (S_H(n) = x(n) for every H), so their outputs are emitted right here, in the natural layout;
+//     G item: the gather for 256 bins (x 1 below N/8, x 3 above) x 16 spectra of a group, low (= long) bins first.
+// Thread 0 of a CTA holds up to one ticket of each queue (fetch-and-add) and runs whichever is runnable, gathers first:
+// a G ticket once ALL T items of its group are complete, a T ticket once the gather of the group that used its ring slot
+// last (g - R) is complete.  A ticket that is not runnable is kept while the other kind of work goes on, so no CTA
+// ever waits inside an item, a slow gather phase throttles the copies without parking CTAs on them (the static
+// "[T(s)][G(s-1)]" order of round 1 parked CTAs on copy items whenever the gathers fell behind), and the ring only has
+// to hold the groups in flight (R slots).  Replacement tickets are drawn while the current item's first loads are in flight.
 //
 // Gather thread = (4 spectra of the group, C = 4 consecutive bins): one 16-byte load per bin and harmonic serves four
-// spectra, the outputs of a thread are four float4 and four 4-byte stores.  Range handling is warp-uniform (a warp owns
-// 32 consecutive bins): harmonic i is in range for every lane iff i (n_hi + 1) <= N.
+// spectra, the outputs of a thread are four float4 and four 4-byte stores; a warp owns 32 consecutive bins.  Range
+// handling is warp-uniform: harmonic i is in range for every lane iff i (n_hi + 1) <= N.  Ring data is read with
+// ordinary (L1-allocating) loads: every CTA's first read of a group follows its own acquire of the group's counter,
+// which invalidates the SM's L1 (SASS: CCTL.IVALL).
 #include "hs_internal.cuh"
 #include "hs_ptx.cuh"
 #include "hs_sync.cuh"
@@ -47,7 +49,6 @@ constexpr int kWarpBins = (32 / kLPR) * C;              // bins per warp
 constexpr int kGTile = kWarps * kWarpBins;              // 256 bins per gather tile
 constexpr int kGSub = 3;                                // tiles per G item above the heavy region (bins >= N/8), 1 below
                                                         // (B200: 1 -> 4.03 ms, 2 -> 3.84, 3 -> 3.76, 4 -> 3.73 with waits, 8 -> 5.2)
-constexpr int kLagDefault = 1;                          // the gather runs `lag` steps behind the copy
 constexpr int kTBins = 512 * 16 / G;                    // bins per T item (32 KiB of input)
 constexpr int kTStride = kTBins + 4;                    // shared-memory row stride (floats) of the copy tile
 constexpr int kMaxRing = 3;
@@ -58,17 +59,22 @@ struct il_params {
     float *sums;
     float *vmax;
     uint8_t *amax;
-    int *ctrl;          // control block (hs_internal.cuh): [0] work counter, [1] error flag, [2..3] waits of T items for
-                        // their ring slot, [4..5] waits of G items for their copies; [16 + g] T items done, [16 + groups + g] G items done
+    int *ctrl;          // control block (hs_internal.cuh): [0] T tickets drawn, [1] error flag, [2] times a CTA found neither of
+                        // its tickets runnable, [3] polls of those, [8] G tickets drawn; [16 + g] T items done, [16 + groups + g] G items done
     unsigned spin_limit;
     int64_t slot_words;
-    int N, B, groups, R, lag, order;
-    int K;              // groups per step (order 1): short spectra need several groups for a step of a few rounds
+    int N, B, groups, R;
     hs_cand_sink sink;
     int nT, nG;         // items per group
     int nHeavy;         // the first nHeavy G items are single tiles (bins below ~N/8: 8 to 32 harmonics per bin)
+    int gsub;           // tiles per G item above the heavy region
     int n_split;        // G items cover bins [0, n_split); T items emit the outputs of [n_split, N)
 };
+
+// Ring data: ordinary weak loads (L1-allocating).  Coherent here because a CTA's first read of a group follows its own
+// acquire of the group's counter (LDG.E.STRONG.GPU + CCTL.IVALL: the SM's L1 is invalidated) and a __syncthreads.
+__device__ __forceinline__ float4 ld_ring(const float4 *p) { return *p; }
+__device__ __forceinline__ float ld_ring(const float *p) { return *p; }
 
 __device__ __forceinline__ float4 ld_stream(const float4 *p)   // read-once input: evict-first in L1 and L2
 {
@@ -78,8 +84,8 @@ __device__ __forceinline__ float4 ld_stream(const float4 *p)   // read-once inpu
 }
 // ------------------------------------------------------------------------------------------------ T item
 // xT[k][g] = x[b0 + g][k] for g < nb, 0 for nb <= g < G, k in [k0, k0 + 512) below N; outputs of the bins >= n_split.
-template <int L, int OUT>
-__device__ __forceinline__ void copy_item(const il_params &p, float *tile, int grp, int k0, float *__restrict__ xT)
+template <int L, int OUT, class F>
+__device__ __forceinline__ void copy_item(const il_params &p, float *tile, int grp, int k0, float *__restrict__ xT, F &redraw)
 {
     const int N = p.N;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -98,6 +104,7 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
             if (g < nb && k < N) v[s][q] = ld_stream(reinterpret_cast<const float4 *>(p.x + (b0 + g) * N + k));
         }
     }
+    redraw();                                           // (thread 0: the next item, while the loads are in flight)
 #pragma unroll
     for (int s = 0; s < SPW; s++) {
         const int g = warp * SPW + s;
@@ -158,20 +165,23 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
 // One tile of 256 bins x 16 spectra.  Thread = (4 spectra, 4 consecutive bins): one 16-byte load per bin and harmonic
 // serves four spectra; a warp owns 32 consecutive bins, and per output row it stores 128 contiguous bytes of maxima
 // and 32 of best levels.
-template <int L, int OUT>
-__device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_cta, const float *__restrict__ xT)
+template <int L, int OUT, class F>
+__device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_cta, const float *xT, F &redraw)
 {
     const int N = p.N;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int q4 = lane & (kLPR - 1);                                           // spectra 4 q4 .. 4 q4 + 3 of the group
     const int n_w = n_cta + warp * kWarpBins;                          // first bin of this warp
     const int n_end = min(N, p.n_split);                               // bins [n_end, N) belong to the T items
-    if (n_w >= n_end) return;                                          // (warp-uniform)
+    if (n_w >= n_end) {                                                // (warp-uniform)
+        redraw();
+        return;
+    }
     const int n0 = n_w + (lane / kLPR) * C;                              // first bin of this thread
     const int n_hi1 = min(n_w + kWarpBins, n_end);                     // one past the warp's last bin
     const bool whole = n_w + kWarpBins <= n_end;                       // every lane's C bins exist
     const int64_t b0 = (int64_t)grp * G + 4 * q4;                      // first of this thread's spectra
-    const float4 *__restrict__ xq = reinterpret_cast<const float4 *>(xT) + q4;   // row k: xq[k * (G / 4)]
+    const float4 *xq = reinterpret_cast<const float4 *>(xT) + q4;                // row k: xq[k * (G / 4)]
     constexpr int RS = G / 4;                                          // float4 per row
 
     float4 S[C];
@@ -219,7 +229,8 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
 
     // harmonic 1
 #pragma unroll
-    for (int k = 0; k < C; k++) S[k] = (whole || n0 + k < N) ? hsptx::ld_cg(xq + (n0 + k) * RS) : zero;
+    for (int k = 0; k < C; k++) S[k] = (whole || n0 + k < N) ? ld_ring(xq + (n0 + k) * RS) : zero;
+    redraw();                                                        // (thread 0: the next item, while the loads are in flight)
     emit(0);
 
     // harmonics i and i + 1, both in range for every lane: no bounds checks, 8 independent 16-byte loads in flight
@@ -228,8 +239,8 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
         float4 a[C], b[C];
 #pragma unroll
         for (int k = 0; k < C; k++) {
-            a[k] = hsptx::ld_cg(xq + (base + k * i) * RS);
-            b[k] = hsptx::ld_cg(xq + (base2 + k * (i + 1)) * RS);
+            a[k] = ld_ring(xq + (base + k * i) * RS);
+            b[k] = ld_ring(xq + (base2 + k * (i + 1)) * RS);
         }
 #pragma unroll
         for (int k = 0; k < C; k++) {
@@ -241,7 +252,7 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
         const int base = i * n0;
         float4 a[C];
 #pragma unroll
-        for (int k = 0; k < C; k++) a[k] = hsptx::ld_cg(xq + (base + k * i) * RS);
+        for (int k = 0; k < C; k++) a[k] = ld_ring(xq + (base + k * i) * RS);
 #pragma unroll
         for (int k = 0; k < C; k++) add(S[k], a[k]);
     };
@@ -251,7 +262,7 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
 #pragma unroll
         for (int k = 0; k < C; k++) {
             const int r = base + k * i;
-            add(S[k], r < N ? hsptx::ld_cg(xq + r * RS) : zero);
+            add(S[k], r < N ? ld_ring(xq + r * RS) : zero);
         }
     };
 
@@ -305,78 +316,71 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
 }
 
 // ------------------------------------------------------------------------------------------------ persistent kernel
+using hssync::kNoTicket;
+using il_tickets = hssync::tickets;
+constexpr int kItemG = 1 << 30;
+
 template <int L, int OUT>
 __global__ void __launch_bounds__(kThreads, 2)
 il_persistent_kernel(const __grid_constant__ il_params p)
 {
     __shared__ __align__(16) float tile[G * kTStride];
     __shared__ int s_item;
-    int *queue = p.ctrl + HS_CTRL_QUEUE;
-    int *doneT = p.ctrl + 16, *doneG = p.ctrl + 16 + p.groups;
-    const int per = p.nT + p.nG, per_step = p.K * per;
-    const int total = ((p.groups + p.K - 1) / p.K + p.lag) * per_step;
-    int lastT = -1, lastG = -1;                                         // thread 0: groups already seen complete
-    if (threadIdx.x == 0) s_item = atomicAdd(queue, 1);
+    il_tickets q;
+    q.tq = p.ctrl + HS_CTRL_QUEUE;
+    q.gq = p.ctrl + 8;
+    q.doneT = p.ctrl + 16;
+    q.doneG = p.ctrl + 16 + p.groups;
+    q.nT = p.nT;
+    q.nG = p.nG;
+    q.R = p.R;
+    q.totalT = p.groups * p.nT;
+    q.totalG = p.groups * p.nG;
+    q.readyT = -1;
+    q.freeG = -1;                                                       // (groups below R have a fresh slot: ts - R <= -1)
+    q.gt = q.tt = kNoTicket;
+    if (threadIdx.x == 0) s_item = q.next(p.ctrl, p.spin_limit, kItemG);
     __syncthreads();
     int item = s_item;
-    while (item < total) {
-        int next = 0;
-        if (threadIdx.x == 0) next = atomicAdd(queue, 1);               // in flight while this item runs
-        // step st = K groups: all their T items first, then the G items of the K groups of step st - lag (order 1);
-        // order 0 (K = 1): T and G items interleaved in proportion nT : nG
-        const int st = item / per_step, r = item - st * per_step;
-        bool isT;
-        int s, idx;                                                     // group and item index inside the group
-        if (p.order) {
-            isT = r < p.K * p.nT;
-            const int r2 = isT ? r : r - p.K * p.nT, n_per = isT ? p.nT : p.nG;
-            const int g = r2 / n_per;
-            idx = r2 - g * n_per;
-            s = (isT ? st : st - p.lag) * p.K + g;
-        } else {
-            const int t_before = (int)(((int64_t)r * p.nT) / per), t_after = (int)(((int64_t)(r + 1) * p.nT) / per);
-            isT = t_after > t_before;
-            idx = isT ? t_before : r - t_before;
-            s = isT ? st : st - p.lag;
-        }
-        if (isT) {                                                      // ---- T item idx of group s
-            if (s < p.groups) {
-                float *xT = p.xT + (int64_t)(s % p.R) * p.slot_words;
-                if (threadIdx.x == 0 && s >= p.R && p.nG > 0 && lastG < s - p.R) {
-                    hssync::wait_count(doneG + (s - p.R), p.nG, p.ctrl, p.ctrl + 2, p.spin_limit);
-                    lastG = s - p.R;
-                }
-                __syncthreads();
-                copy_item<L, OUT>(p, tile, s, idx * kTBins, xT);
-                __syncthreads();                                        // all stores of the CTA are ordered before ...
-                if (threadIdx.x == 0) {
-                    __threadfence();                                    // ... thread 0's release at gpu scope
-                    atomicAdd(doneT + s, 1);
-                }
+    while (item != kNoTicket) {
+        // the ticket that replaces the one being run is drawn once this item's first loads are issued
+        auto redraw = [&]() {
+            if (threadIdx.x == 0) {
+                q.draw_g();
+                q.draw_t();
             }
-        } else if (s >= 0 && s < p.groups) {                            // ---- G item idx of group s
-            const int grp = s;
+        };
+        if (!(item & kItemG)) {                                         // ---- T item
+            const int s = item / p.nT, idx = item - s * p.nT;
+            float *xT = p.xT + (int64_t)(s % p.R) * p.slot_words;
+            copy_item<L, OUT>(p, tile, s, idx * kTBins, xT, redraw);
+            __syncthreads();                                            // all stores of the CTA are ordered before ...
+            if (threadIdx.x == 0) {
+                __threadfence();                                        // ... thread 0's release at gpu scope
+                atomicAdd(q.doneT + s, 1);
+            }
+        } else {                                                        // ---- G item
+            const int gi = item & (kItemG - 1);
+            const int grp = gi / p.nG, qi = gi - grp * p.nG;
             const float *xT = p.xT + (int64_t)(grp % p.R) * p.slot_words;
-            if (threadIdx.x == 0 && lastT < grp) {
-                hssync::wait_count(doneT + grp, p.nT, p.ctrl, p.ctrl + 4, p.spin_limit);
-                lastT = grp;
-            }
-            __syncthreads();
-            const int q = idx;
-            if (q < p.nHeavy) {
-                gather_item<L, OUT>(p, grp, q * kGTile, xT);
+            if (qi < p.nHeavy) {
+                gather_item<L, OUT>(p, grp, qi * kGTile, xT, redraw);
             } else {
+                auto nothing = []() {};
 #pragma unroll 1
-                for (int sub = 0; sub < kGSub; sub++)
-                    gather_item<L, OUT>(p, grp, (p.nHeavy + (q - p.nHeavy) * kGSub + sub) * kGTile, xT);
+                for (int sub = 0; sub < p.gsub; sub++) {
+                    const int t = p.nHeavy + (qi - p.nHeavy) * p.gsub + sub;
+                    if (sub == 0) gather_item<L, OUT>(p, grp, t * kGTile, xT, redraw);
+                    else gather_item<L, OUT>(p, grp, t * kGTile, xT, nothing);
+                }
             }
-            __syncthreads();
+            __syncthreads();                                            // every load of the slot has returned
             if (threadIdx.x == 0) {
                 __threadfence();
-                atomicAdd(doneG + grp, 1);
+                atomicAdd(q.doneG + grp, 1);
             }
         }
-        if (threadIdx.x == 0) s_item = next;
+        if (threadIdx.x == 0) s_item = q.next(p.ctrl, p.spin_limit, kItemG);
         __syncthreads();                                                // s_item and the tile are reused
         item = s_item;
         __syncthreads();
@@ -384,42 +388,42 @@ il_persistent_kernel(const __grid_constant__ il_params p)
 }
 
 struct il_sched {
-    int groups, R, lag, K, nT, nG, nHeavy, n_split;
+    int groups, R, nT, nG, nHeavy, gsub, n_split;
     int64_t slot_words;
 };
+constexpr int kCtasPerSm = 2;                                           // (__launch_bounds__ of the kernel)
 
 il_sched make_sched(const hs_plan *p, int64_t batch)
 {
     il_sched s{};
     const int N = (int)p->nbins;
     s.groups = (int)((batch + G - 1) / G);
-    int ring = kMaxRing;
-    s.lag = kLagDefault;
-    ring = hs_knob("HS_IL_RING", ring);
-    s.lag = hs_knob("HS_IL_LAG", s.lag);
-    if (s.lag < 1) s.lag = 1;
-    if (ring < s.lag + 2) ring = s.lag + 2;                            // a slot is rewritten only after its gather was handed out
     s.nT = (N + kTBins - 1) / kTBins;
     // bins n >= N/2 have S_H(n) = x(n): the T items emit them.  The split is a multiple of the T tile.
     const int half = (N + 1) / 2;
     int split = (half + kTBins - 1) / kTBins * kTBins;
     if (p->Hmax == 1) split = 0;                                       // nothing to gather at all
-    if (split > N) split = (N + kGTile - 1) / kGTile * kGTile;          // (only spectra shorter than a T tile)
+    const int gt = kGTile;
+    if (split > N) split = (N + gt - 1) / gt * gt;                      // (only spectra shorter than a T tile)
     s.n_split = split;
-    const int tiles = (((split < N) ? split : N) + kGTile - 1) / kGTile;
-    s.nHeavy = (N / 8 + kGTile - 1) / kGTile;
+    const int tiles = (((split < N) ? split : N) + gt - 1) / gt;
+    s.nHeavy = (N / 8 + gt - 1) / gt;
     if (s.nHeavy > tiles) s.nHeavy = tiles;
-    s.nG = s.nHeavy + (tiles - s.nHeavy + kGSub - 1) / kGSub;
+    s.gsub = hs_knob("HS_IL_GSUB", kGSub);
+    if (s.gsub < 1) s.gsub = 1;
+    s.nG = s.nHeavy + (tiles - s.nHeavy + s.gsub - 1) / s.gsub;
     s.slot_words = ((int64_t)N * G + 63) & ~(int64_t)63;
-    // groups per step: a step has to be ~2.6 rounds of the resident CTAs (2 per SM) or its dependences are exercised;
-    // one group of 2^18-bin spectra is that long, shorter spectra take several (the ring stays 48 MiB)
-    const int per = s.nT + s.nG;
-    int K = (int)((2.6 * 2 * p->sm_count + per / 2) / per);
-    K = hs_knob("HS_IL_K", K);
-    if (K < 1 || hs_knob("HS_IL_ORDER", 1) != 1) K = 1;
-    s.K = K;
-    ring *= K;
-    s.R = s.groups < ring ? s.groups : ring;
+    // Ring slots: the copies run ahead of the gathers by at most R groups.  Three 16 MiB slots (2^18 bins) keep the
+    // resident CTAs busy; shorter spectra need more groups in flight for that (about two items per resident CTA),
+    // within the same 48 MiB.
+    const int64_t slot_bytes = s.slot_words * 4;
+    int64_t R = (2 * (int64_t)kCtasPerSm * p->sm_count + s.nT - 1) / s.nT + 1;
+    const int64_t cap = ((int64_t)48 << 20) / slot_bytes;
+    if (R > cap) R = cap;
+    if (R < kMaxRing) R = kMaxRing;
+    R = hs_knob("HS_IL_RING", (int)R);
+    if (R < 2) R = 2;
+    s.R = (int)(s.groups < R ? s.groups : R);
     return s;
 }
 
@@ -442,20 +446,18 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.B = (int)batch;
     prm.groups = s.groups;
     prm.R = s.R;
-    prm.lag = s.lag;
-    prm.K = s.K;
-    prm.order = hs_knob("HS_IL_ORDER", 1);
     prm.spin_limit = hs_spin_limit();
     prm.nT = s.nT;
     prm.nG = s.nG;
     prm.nHeavy = s.nHeavy;
+    prm.gsub = s.gsub;
     prm.n_split = s.n_split;
     auto kern = il_persistent_kernel<L, OUT>;
     int occ = 0;                                                        // (per device: asked on every launch)
     HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, 0));
     const int ctas_per_sm = occ > 0 ? occ : 1;
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(s.groups), stream));
-    const int64_t total = (int64_t)((s.groups + s.K - 1) / s.K + s.lag) * s.K * (s.nT + s.nG);
+    const int64_t total = (int64_t)s.groups * (s.nT + s.nG);
     const int64_t slots = (int64_t)p->sm_count * ctas_per_sm;
     kern<<<(unsigned)(total < slots ? total : slots), kThreads, 0, stream>>>(prm);
     HS_CUDA_OK(cudaGetLastError());
@@ -477,7 +479,6 @@ int by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
 int by_level(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
     switch (p->L) {
-        case 1: return by_out<1>(p, buf, batch, ws, stream);
         case 2: return by_out<2>(p, buf, batch, ws, stream);
         case 3: return by_out<3>(p, buf, batch, ws, stream);
         case 4: return by_out<4>(p, buf, batch, ws, stream);
@@ -493,9 +494,9 @@ int by_level(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, c
 bool hs_interleaved_supported(const hs_plan *p)
 {
     if (p->variant != HS_FREQBIN) return false;
-    if (p->nbins > ((int64_t)1 << 18)) return false;
+    if (p->Hmax < 2 || p->nbins > ((int64_t)1 << 18)) return false;
     const il_sched s = make_sched(p, p->batch);
-    return ((int64_t)(s.groups + s.K - 1) / s.K + s.lag) * s.K * (s.nT + s.nG) < ((int64_t)1 << 30);
+    return (int64_t)s.groups * (s.nT > s.nG ? s.nT : s.nG) < ((int64_t)1 << 30);   // (item codes: bit 30 marks a G item)
 }
 
 size_t hs_interleaved_workspace_bytes(const hs_plan *p, int64_t batch)

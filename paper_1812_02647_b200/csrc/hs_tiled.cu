@@ -16,6 +16,7 @@ bool grouped(const hs_plan *p)
     if (max_gather(p)) return false;
     if (p->algo_req == HS_ALGO_TWOPHASE || p->algo_req == HS_ALGO_GATHER) return false;
     if (p->variant == HS_FREQBIN && p->algo_req != HS_ALGO_GROUPED) return false;
+    if (p->variant == HS_GREEDY) return false;
     return hs_grouped_supported(p);
 }
 // Max otherwise runs two-phase; freq-bin runs two-phase only when asked to (HS_ALGO_TWOPHASE).
