@@ -63,9 +63,20 @@ enum hs_algo {
     HS_ALGO_TWOPHASE = 3, /* eqs. 2-3 only: the two-phase kernel (for eq. 2 the same as HS_ALGO_TILED)              */
     HS_ALGO_GATHER = 4,   /* eqs. 3-4 only: the range-skipping gather straight from x (no workspace); what
                              HS_ALGO_TILED itself uses for spectra too long for the interleaved group copy           */
-    HS_ALGO_GROUPED = 5   /* eqs. 2-3 only, Hmax >= 2, nbins <= 2^23: two phases per spectrum by a static group of co-resident CTAs, the
+    HS_ALGO_GROUPED = 5,  /* eqs. 2-3 only, Hmax >= 2, nbins <= 2^23: two phases per spectrum by a static group of co-resident CTAs, the
                              per-harmonic arrays of a spectrum live in one L2-resident workspace slot per group
                              (cooperative launch)                                                                   */
+    HS_ALGO_GENERAL = 6   /* what plans of hs_plan_create_ex (every integer H, printed window) and hs_plan_create_2d
+                             resolve to: one thread per output, no workspace; not selectable for other plans        */
+};
+/* hs_plan_create_ex options */
+enum hs_levels {
+    HS_LEVELS_DYADIC = 0, /* H = 1, 2, 4, .., Hmax (BASELINE.json north_star)                                        */
+    HS_LEVELS_ALL = 1     /* every integer H = 1 .. Hmax, Hmax <= 64 ("an increasing number of harmonics") */
+};
+enum hs_window {
+    HS_WINDOW_C2 = 0,     /* eq. 2 window j = 0 .. i-1 (CONVENTIONS.md C2: h_1(n) = x(n))                             */
+    HS_WINDOW_PRINTED = 1 /* eq. 2 window exactly as printed, j = 1 .. i: h_1(n) = x(n + 1)             */
 };
 
 /*
@@ -83,6 +94,29 @@ enum hs_algo {
  * Returns NULL on error: HS_ERR_INVALID_ARG (checked first), HS_ERR_UNSUPPORTED, HS_ERR_CUDA.
  */
 hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode);
+
+/*
+ * hs_plan_create_ex — the variants of the paper's own description beyond the dyadic default:
+ *   levels   HS_LEVELS_ALL: partial sums for EVERY integer H = 1..Hmax, 1 <= Hmax <= 64.  Level index l = H - 1, so
+ *            sums is [batch][Hmax][nbins], argmax holds H - 1, hs_plan_levels returns Hmax.  eq. 1 uses the nearest
+ *            bin, half up, for any H: x(floor((2 n i + H) / (2 H))) (= CONVENTIONS.md C1 for even H); h_H = S_H / sqrt(H).
+ *            nbins <= 2^24.  HS_LEVELS_DYADIC with HS_WINDOW_C2 is exactly hs_plan_create.
+ *   window   HS_WINDOW_PRINTED (HS_MAX only, else HS_ERR_INVALID_ARG): eq. 2 with 1 <= j <= i as the paper prints it.
+ * Such plans resolve to HS_ALGO_GENERAL (no workspace); hs_plan_set_algo accepts only HS_ALGO_AUTO for them.
+ */
+hs_plan *hs_plan_create_ex(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode, int levels, int window);
+
+/*
+ * hs_plan_create_2d — the two-dimensional harmonic sum over the f - fdot plane of a Fourier-domain acceleration search
+ * (reading R-2D of DESIGN.md section 16: the paper gives no equation).
+ * One batch entry is a plane x[nz][nbins] (row-major); row zi holds drift z = zi - (nz-1)/2, nz odd, 1 <= nz <= 4095.
+ * Harmonic i of a signal at (bin n, drift z) sits at (n i/H, z i/H):
+ *     HS_STANDARD  S_H(n, z) = sum_{i=1..H} x(floor((z i + H/2)/H), floor((n i + H/2)/H))     (floor toward -infinity)
+ *     HS_FREQBIN   S_H(n, z) = sum_{i=1..H} x~(i z, i n)                                       (0 outside the plane)
+ * (other variants: HS_ERR_INVALID_ARG), dyadic levels, h_H = S_H / sqrt(H).  Layouts: x [batch][nz][nbins],
+ * sums [batch][L][nz][nbins], max / argmax [batch][nz][nbins].  Execute with hs_execute / hs_execute_host.
+ */
+hs_plan *hs_plan_create_2d(int64_t nbins, int64_t nz, int64_t batch, int Hmax, int variant, int out_mode);
 
 /*
  * hs_execute — enqueue the transform on `stream` (a cudaStream_t; NULL = the legacy default stream) and return

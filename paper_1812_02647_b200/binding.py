@@ -15,7 +15,11 @@ LIB_PATH = os.path.join(_HERE, os.path.basename(os.environ.get("HS_LIBRARY", "li
 
 HS_STANDARD, HS_MAX, HS_FREQBIN, HS_GREEDY = 0, 1, 2, 3
 HS_OUT_FULL, HS_OUT_REDUCED, HS_OUT_BOTH = 1, 2, 3
-HS_ALGO_AUTO, HS_ALGO_DIRECT, HS_ALGO_TILED, HS_ALGO_TWOPHASE, HS_ALGO_GATHER, HS_ALGO_GROUPED = 0, 1, 2, 3, 4, 5
+HS_ALGO_AUTO, HS_ALGO_DIRECT, HS_ALGO_TILED, HS_ALGO_TWOPHASE, HS_ALGO_GATHER, HS_ALGO_GROUPED, HS_ALGO_GENERAL = 0, 1, 2, 3, 4, 5, 6
+HS_LEVELS_DYADIC, HS_LEVELS_ALL = 0, 1
+HS_WINDOW_C2, HS_WINDOW_PRINTED = 0, 1
+LEVELS = {"dyadic": HS_LEVELS_DYADIC, "all": HS_LEVELS_ALL}
+WINDOWS = {"c2": HS_WINDOW_C2, "printed": HS_WINDOW_PRINTED}
 (HS_OK, HS_ERR_INVALID_ARG, HS_ERR_NULL_POINTER, HS_ERR_MISALIGNED, HS_ERR_UNSUPPORTED, HS_ERR_WORKSPACE, HS_ERR_CUDA,
  HS_ERR_DEVICE_TIMEOUT) = range(8)
 VARIANTS = {"standard": HS_STANDARD, "max": HS_MAX, "freqbin": HS_FREQBIN, "greedy": HS_GREEDY}
@@ -31,6 +35,8 @@ lib = ctypes.CDLL(LIB_PATH)
 _i64, _p, _int, _sz = ctypes.c_int64, ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
 _SIGS = {
     "hs_plan_create": ([_i64, _i64, _int, _int, _int], _p),
+    "hs_plan_create_ex": ([_i64, _i64, _int, _int, _int, _int, _int], _p),
+    "hs_plan_create_2d": ([_i64, _i64, _i64, _int, _int, _int], _p),
     "hs_execute": ([_p, _p, _p, _p, _p, _p], _int),
     "hs_destroy": ([_p], _int),
     "hs_last_error": ([], _int),
@@ -84,12 +90,33 @@ def hs_plan_create(nbins: int, batch: int, Hmax: int, variant, out_mode):
     return Plan(h, int(nbins), int(batch), int(Hmax), v, o)
 
 
+def hs_plan_create_ex(nbins: int, batch: int, Hmax: int, variant, out_mode, levels="dyadic", window="c2"):
+    v = VARIANTS[variant] if isinstance(variant, str) else int(variant)
+    o = OUT_MODES[out_mode] if isinstance(out_mode, str) else int(out_mode)
+    lv = LEVELS[levels] if isinstance(levels, str) else int(levels)
+    w = WINDOWS[window] if isinstance(window, str) else int(window)
+    h = lib.hs_plan_create_ex(int(nbins), int(batch), int(Hmax), v, o, lv, w)
+    if not h:
+        raise HsError(lib.hs_last_error(), "hs_plan_create_ex")
+    return Plan(h, int(nbins), int(batch), int(Hmax), v, o)
+
+
+def hs_plan_create_2d(nbins: int, nz: int, batch: int, Hmax: int, variant, out_mode):
+    v = VARIANTS[variant] if isinstance(variant, str) else int(variant)
+    o = OUT_MODES[out_mode] if isinstance(out_mode, str) else int(out_mode)
+    h = lib.hs_plan_create_2d(int(nbins), int(nz), int(batch), int(Hmax), v, o)
+    if not h:
+        raise HsError(lib.hs_last_error(), "hs_plan_create_2d")
+    return Plan(h, int(nbins), int(batch), int(Hmax), v, o, nz=int(nz))
+
+
 class Plan:
     """Owns one hs_plan handle plus the torch tensors lent to it as workspace/staging."""
 
-    def __init__(self, handle, nbins, batch, Hmax, variant, out_mode):
+    def __init__(self, handle, nbins, batch, Hmax, variant, out_mode, nz=1):
         self.handle = ctypes.c_void_p(handle)
         self.nbins, self.batch, self.Hmax, self.variant, self.out_mode = nbins, batch, Hmax, variant, out_mode
+        self.nz = nz
         self.levels = lib.hs_plan_levels(self.handle)
         self._ws = None
         self._staging = None
@@ -172,13 +199,14 @@ class Plan:
         """Allocate the outputs the plan's out_mode asks for, execute, return (sums, max, argmax) (None if absent)."""
         import torch
         assert d_x.is_cuda and d_x.dtype == torch.float32 and d_x.is_contiguous()
-        assert tuple(d_x.shape) == (self.batch, self.nbins)
+        row = (self.nbins,) if self.nz == 1 else (self.nz, self.nbins)     # one batch entry: a spectrum or a plane
+        assert tuple(d_x.shape) == (self.batch,) + row
         sums = vmax = amax = None
         if self.out_mode & HS_OUT_FULL:
-            sums = torch.empty((self.batch, self.levels, self.nbins), dtype=torch.float32, device=d_x.device)
+            sums = torch.empty((self.batch, self.levels) + row, dtype=torch.float32, device=d_x.device)
         if self.out_mode & HS_OUT_REDUCED:
-            vmax = torch.empty((self.batch, self.nbins), dtype=torch.float32, device=d_x.device)
-            amax = torch.empty((self.batch, self.nbins), dtype=torch.uint8, device=d_x.device)
+            vmax = torch.empty((self.batch,) + row, dtype=torch.float32, device=d_x.device)
+            amax = torch.empty((self.batch,) + row, dtype=torch.uint8, device=d_x.device)
         self.ensure_workspace(d_x.device)
         self.hs_execute(d_x, sums, vmax, amax, stream)
         return sums, vmax, amax

@@ -22,9 +22,12 @@ int levels_of(int Hmax)
     }
 }
 
+bool is_general(const hs_plan *p) { return p->nz > 1 || p->levels_mode != HS_LEVELS_DYADIC || p->window != HS_WINDOW_C2; }
+
 void resolve_algo(hs_plan *p)
 {
-    if (p->algo_req == HS_ALGO_DIRECT) p->algo = HS_ALGO_DIRECT;
+    if (is_general(p)) p->algo = HS_ALGO_GENERAL;
+    else if (p->algo_req == HS_ALGO_DIRECT) p->algo = HS_ALGO_DIRECT;
     else if (p->algo_req == HS_ALGO_TILED || p->algo_req == HS_ALGO_TWOPHASE || p->algo_req == HS_ALGO_GATHER ||
              p->algo_req == HS_ALGO_GROUPED)
         p->algo = HS_ALGO_TILED;
@@ -73,6 +76,7 @@ int check_buffers(const hs_plan *p, const void *x, const void *sums, const void 
 int launch_family(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
     if (p->algo == HS_ALGO_TILED) return hs_launch_tiled(p, buf, batch, ws, stream);
+    if (p->algo == HS_ALGO_GENERAL) return hs_launch_general(p, buf, batch, ws, stream);
     return hs_launch_direct(p, buf, batch, ws, stream);
 }
 
@@ -85,7 +89,7 @@ struct slab_layout {
 slab_layout layout_of(const hs_plan *p, int64_t slab)
 {
     slab_layout s{};
-    const size_t bins = (size_t)slab * (size_t)p->nbins;
+    const size_t bins = (size_t)slab * (size_t)p->nbins * (size_t)p->nz;
     s.x = round_up(bins * 4, 256);
     s.sums = (p->out_mode & HS_OUT_FULL) ? round_up(bins * 4 * p->L, 256) : 0;
     s.vmax = (p->out_mode & HS_OUT_REDUCED) ? round_up(bins * 4, 256) : 0;
@@ -119,12 +123,19 @@ const char *hs_error_string(int code)
 
 const char *hs_version(void) { return "hs 0.2 (sm_100a)"; }
 
-hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode)
+static hs_plan *create_plan(int64_t nbins, int64_t nz, int64_t batch, int Hmax, int variant, int out_mode, int levels, int window)
 {
-    const int L = levels_of(Hmax);
-    if (nbins < 4 || nbins > ((int64_t)1 << 25) || (nbins % 4) != 0 || batch < 1 || L < 0 ||
-        variant < HS_STANDARD || variant > HS_GREEDY || out_mode < HS_OUT_FULL || out_mode > HS_OUT_BOTH ||
-        batch > ((int64_t)1 << 40) / nbins || batch > (int64_t)0x7fffffff) {
+    const bool all = levels == HS_LEVELS_ALL;
+    const int L = all ? Hmax : levels_of(Hmax);
+    bool bad = nbins < 4 || nbins > ((int64_t)1 << 25) || (nbins % 4) != 0 || batch < 1 || L < 1 ||
+               variant < HS_STANDARD || variant > HS_GREEDY || out_mode < HS_OUT_FULL || out_mode > HS_OUT_BOTH ||
+               nz < 1 || batch > ((int64_t)1 << 40) / (nbins * (nz > 0 ? nz : 1)) || batch > (int64_t)0x7fffffff;
+    bad = bad || (levels != HS_LEVELS_DYADIC && levels != HS_LEVELS_ALL) || (window != HS_WINDOW_C2 && window != HS_WINDOW_PRINTED);
+    bad = bad || (all && (Hmax < 1 || Hmax > 64 || nbins > ((int64_t)1 << 24)));
+    bad = bad || (window == HS_WINDOW_PRINTED && variant != HS_MAX);
+    bad = bad || (nz > 1 && ((nz % 2) == 0 || nz > 4095 || all || window != HS_WINDOW_C2 ||
+                             (variant != HS_STANDARD && variant != HS_FREQBIN)));
+    if (bad) {
         hs_set_error(HS_ERR_INVALID_ARG);
         return nullptr;
     }
@@ -152,6 +163,9 @@ hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int
     }
     p->nbins = nbins;
     p->batch = batch;
+    p->nz = nz;
+    p->levels_mode = levels;
+    p->window = window;
     p->Hmax = Hmax;
     p->L = L;
     p->variant = variant;
@@ -166,6 +180,25 @@ hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int
     p->lanes_ready = false;
     resolve_algo(p);
     return p;
+}
+
+hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode)
+{
+    return create_plan(nbins, 1, batch, Hmax, variant, out_mode, HS_LEVELS_DYADIC, HS_WINDOW_C2);
+}
+
+hs_plan *hs_plan_create_ex(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode, int levels, int window)
+{
+    return create_plan(nbins, 1, batch, Hmax, variant, out_mode, levels, window);
+}
+
+hs_plan *hs_plan_create_2d(int64_t nbins, int64_t nz, int64_t batch, int Hmax, int variant, int out_mode)
+{
+    if (nz < 1 || (nz % 2) == 0 || (variant != HS_STANDARD && variant != HS_FREQBIN)) {
+        hs_set_error(HS_ERR_INVALID_ARG);
+        return nullptr;
+    }
+    return create_plan(nbins, nz, batch, Hmax, variant, out_mode, HS_LEVELS_DYADIC, HS_WINDOW_C2);
 }
 
 int hs_destroy(hs_plan *p)
@@ -190,6 +223,7 @@ int hs_plan_set_algo(hs_plan *p, int algo)
 {
     if (!p) HS_FAIL(HS_ERR_NULL_POINTER);
     if (algo < HS_ALGO_AUTO || algo > HS_ALGO_GROUPED) HS_FAIL(HS_ERR_INVALID_ARG);
+    if (is_general(p) && algo != HS_ALGO_AUTO) HS_FAIL(HS_ERR_INVALID_ARG);      // (one family: HS_ALGO_GENERAL)
     if ((algo == HS_ALGO_TWOPHASE || algo == HS_ALGO_GROUPED) && p->variant != HS_MAX && p->variant != HS_FREQBIN)
         HS_FAIL(HS_ERR_INVALID_ARG);
     if (algo == HS_ALGO_GATHER && p->variant != HS_GREEDY && p->variant != HS_FREQBIN &&
@@ -233,6 +267,7 @@ int hs_plan_launches(const hs_plan *p)
 {
     if (!p) return -1;
     if (p->algo == HS_ALGO_TILED) return hs_tiled_launches(p, p->batch);
+    if (p->algo == HS_ALGO_GENERAL) return (int)((p->batch + 65534) / 65535);
     const int64_t tiles = (p->nbins + 255) / 256;
     const int64_t max_spectra = ((int64_t)1 << 30) / tiles;
     return (int)((p->batch + max_spectra - 1) / max_spectra);
@@ -254,7 +289,7 @@ int hs_execute_candidates(const hs_plan *p, const float *d_x, float threshold, h
                           unsigned long long *d_count, void *stream)
 {
     if (!p || !d_x || !d_count || (!d_cand && capacity > 0)) HS_FAIL(HS_ERR_NULL_POINTER);
-    if (p->out_mode != HS_OUT_REDUCED || capacity < 0 || !(threshold == threshold)) HS_FAIL(HS_ERR_INVALID_ARG);
+    if (p->out_mode != HS_OUT_REDUCED || capacity < 0 || !(threshold == threshold) || p->nz > 1) HS_FAIL(HS_ERR_INVALID_ARG);
     if (!aligned(d_x, 16) || !aligned(d_cand, 16) || !aligned(d_count, 8)) HS_FAIL(HS_ERR_MISALIGNED);
     const int rcd = check_device(p);
     if (rcd != HS_OK) return rcd;
@@ -337,13 +372,13 @@ int hs_execute_host(hs_plan *p, const float *h_x, float *h_sums, float *h_max, u
     const slab_layout lay = layout_of(p, p->slab);
     if (p->staging_bytes < lay.total * HS_HOST_LANES) HS_FAIL(HS_ERR_WORKSPACE);   // (sized for another algorithm)
     p->n_last_ctrl = 0;
-    const int64_t N = p->nbins;
+    const int64_t N = p->nbins * p->nz;
     HS_CUDA_OK(cudaEventRecord(p->fork, user));
     for (int i = 0; i < HS_HOST_LANES; i++) HS_CUDA_OK(cudaStreamWaitEvent(p->lane_stream[i], p->fork, 0));
     int lane = 0;
     for (int64_t b0 = 0; b0 < p->batch; b0 += p->slab, lane = (lane + 1) % HS_HOST_LANES) {
         const int64_t nb = (p->batch - b0 < p->slab) ? p->batch - b0 : p->slab;
-        const size_t bins = (size_t)nb * (size_t)N;
+        const size_t bins = (size_t)nb * (size_t)N;                     // (N = elements per batch entry)
         char *base = static_cast<char *>(p->staging) + (size_t)lane * lay.total;
         float *dx = reinterpret_cast<float *>(base);
         float *dsums = lay.sums ? reinterpret_cast<float *>(base + lay.x) : nullptr;

@@ -38,6 +38,9 @@ inline unsigned hs_spin_limit() { return (unsigned)hs_knob("HS_SPIN_LIMIT", (int
 
 struct hs_plan {
     int64_t nbins, batch;
+    int64_t nz;        // rows of the f - fdot plane per batch entry (1: the one-dimensional sum)
+    int levels_mode;   // enum hs_levels
+    int window;        // enum hs_window (eq. 2 only)
     int Hmax, L, variant, out_mode;
     int algo_req;  // what the caller asked for (enum hs_algo)
     int algo;      // resolved family, never AUTO
@@ -95,6 +98,7 @@ struct hs_buffers {
     hs_cand_sink sink;
 };
 int hs_launch_direct(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
+int hs_launch_general(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);   // hs_general.cu
 int hs_launch_tiled(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
 size_t hs_tiled_workspace_bytes(const hs_plan *p, int64_t batch);
 int hs_tiled_launches(const hs_plan *p, int64_t batch);

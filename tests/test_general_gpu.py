@@ -1,0 +1,200 @@
+"""Parity of the SURVEY.md section 8(f) rows on the GPU (through the C ABI) with oracle/hs_oracle_ext.c: every integer H
+up to 64, eq. 2 with the window as printed, the two-dimensional sum over the f - fdot plane, and the fused power-spectrum
+front end.  Tolerances as CONVENTIONS.md C10."""
+import numpy as np
+import pytest
+import torch
+
+import workloads as W
+from parity import argmax_from_levels, check_argmax, check_sums
+
+pytestmark = pytest.mark.gpu
+VARIANTS = ["standard", "max", "freqbin", "greedy"]
+
+
+@pytest.fixture(scope="module")
+def hs():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1812_02647_b200 import build
+    build.build()
+    import paper_1812_02647_b200.binding as binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ext():
+    from oracle import ext as _ext
+    _ext.build()
+    return _ext
+
+
+def compare(plan, got, ref, what, x_np=None, printed=False):
+    sums, vmax, amax = got
+    if sums is not None:
+        check_sums(sums.cpu().numpy(), ref["sums"], what + " sums")
+        if x_np is not None and not printed:
+            np.testing.assert_array_equal(sums[:, 0].cpu().numpy(), x_np)          # h_1 = x bit-exactly
+    if vmax is not None:
+        check_sums(vmax.cpu().numpy(), ref["max"], what + " max")
+        check_argmax(amax.cpu().numpy(), ref["argmax"], ref["second"], ref["gap"], ref["max"], what + " argmax")
+    if sums is not None and vmax is not None:
+        pick = torch.gather(sums, 1, amax.long().unsqueeze(1)).squeeze(1)
+        assert torch.equal(pick, vmax), what + " max != sums[argmax]"
+
+
+# ------------------------------------------------------------------------------------------ every integer H, printed window
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_every_integer_H_whole_batch(hs, ext, variant):
+    rng = np.random.default_rng(41)
+    for N, B, Hmax in ((4, 1, 64), (100, 2, 64), (4100, 2, 64), (20000, 3, 24), (1 << 15, 2, 7), (2052, 5, 1)):
+        x, _ = W.comb_batch_numpy(2, list(range(B)), N, 0.5, 5.0, max(6.0, N / 40), 0.10) if N >= 256 else \
+            ((rng.standard_exponential((B, N)) - 1).astype(np.float32), None)
+        d_x = torch.from_numpy(x).cuda()
+        for out_mode in ("both", "reduced", "full"):
+            plan = hs.hs_plan_create_ex(N, B, Hmax, variant, out_mode, "all", "c2")
+            assert plan.levels == Hmax and plan.algo == hs.HS_ALGO_GENERAL and plan.workspace_bytes() == 0
+            got = plan.run(d_x)
+            plan.device_status()
+            ref = ext.harmonic_sum_all(x, Hmax, variant, want_jpath=(variant == "greedy"))
+            compare(plan, got, ref, f"all-H {variant}/{out_mode}/N={N}/Hmax={Hmax}", x)
+            if variant == "greedy" and out_mode == "full":
+                d_j = torch.empty((B, Hmax, N), dtype=torch.uint8, device="cuda")
+                plan.hs_debug_greedy_paths(d_x, d_j)
+                torch.cuda.synchronize()
+                np.testing.assert_array_equal(d_j.cpu().numpy(), ref["jpath"])
+            plan.hs_destroy()
+
+
+def test_every_integer_H_degenerate_spectra_and_ties(hs, ext):
+    N = 3000
+    rng = np.random.default_rng(42)
+    cases = [np.zeros(N), -np.ones(N), np.ones(N), np.arange(N), np.arange(N)[::-1], rng.integers(-2, 3, N)]
+    x = np.stack(cases).astype(np.float32)
+    d_x = torch.from_numpy(x).cuda()
+    for variant in VARIANTS:
+        plan = hs.hs_plan_create_ex(N, len(cases), 48, variant, "both", "all", "c2")
+        compare(plan, plan.run(d_x), ext.harmonic_sum_all(x, 48, variant), f"all-H degenerate {variant}", x)
+
+
+def test_eq2_window_as_printed(hs, ext):
+    for N, B, Hmax, levels in ((20000, 3, 32, "dyadic"), (4100, 2, 64, "all"), (100, 1, 16, "dyadic"), (1 << 15, 2, 40, "all")):
+        x, _ = W.comb_batch_numpy(2, list(range(B)), N, 1.0, 5.0, max(6.0, N / 40), 0.10) if N >= 256 else \
+            ((np.random.default_rng(43).standard_exponential((B, N)) - 1).astype(np.float32), None)
+        d_x = torch.from_numpy(x).cuda()
+        plan = hs.hs_plan_create_ex(N, B, Hmax, "max", "both", levels, "printed")
+        sums, vmax, amax = plan.run(d_x)
+        torch.cuda.synchronize()
+        ref = ext.harmonic_sum_all(x, Hmax, "max", "printed")
+        if levels == "dyadic":                                   # the dyadic levels of the all-H oracle
+            pick = [h - 1 for h in (1, 2, 4, 8, 16, 32, 64) if h <= Hmax]
+            ref_sums = ref["sums"][:, pick]
+            best, second, gap, m = argmax_from_levels(np.moveaxis(ref_sums, 1, -1))
+            ref = {"sums": ref_sums, "max": m, "argmax": best, "second": second, "gap": gap}
+        compare(plan, (sums, vmax, amax), ref, f"printed window N={N} Hmax={Hmax} {levels}", printed=True)
+        shifted = np.concatenate([x[:, 1:], np.zeros((B, 1), np.float32)], axis=1)          # h_1(n) = x(n + 1)
+        np.testing.assert_array_equal(sums[:, 0].cpu().numpy(), shifted)
+    with pytest.raises(hs.HsError) as e:
+        hs.hs_plan_create_ex(4096, 1, 32, "greedy", "full", "dyadic", "printed")
+    assert e.value.code == hs.HS_ERR_INVALID_ARG
+
+
+def test_general_plans_reject_other_families_and_bad_arguments(hs):
+    plan = hs.hs_plan_create_ex(4096, 2, 64, "freqbin", "reduced", "all", "c2")
+    for algo in ("direct", "tiled", "gather"):
+        with pytest.raises(hs.HsError):
+            plan.set_algo(algo)
+    plan.set_algo("auto")
+    for bad in ((4096, 1, 65, "max", "full", "all", "c2"), (4096, 1, 0, "max", "full", "all", "c2"),
+                (1 << 25, 1, 8, "max", "reduced", "all", "c2")):
+        with pytest.raises(hs.HsError) as e:
+            hs.hs_plan_create_ex(*bad)
+        assert e.value.code == hs.HS_ERR_INVALID_ARG
+    for bad in ((4096, 4, 1, 32, "standard", "full"), (4096, 5, 1, 32, "max", "full"), (4096, 5, 1, 3, "standard", "full")):
+        with pytest.raises(hs.HsError) as e:
+            hs.hs_plan_create_2d(*bad)
+        assert e.value.code == hs.HS_ERR_INVALID_ARG
+    d = hs.hs_plan_create_ex(4096, 1, 32, "max", "full", "dyadic", "c2")          # the plain plan: not general
+    assert d.algo != hs.HS_ALGO_GENERAL
+
+
+def test_every_integer_H_sampled_at_bench_size(hs, ext):
+    """The shape bench.py --workload allh times (256 spectra x 2^18 bins, Hmax 64, reduced), sampled outputs."""
+    B, N, Hmax = 256, 1 << 18, 64
+    d_x = W.exp_noise_torch(B, N, 7, "cuda")
+    rng = np.random.default_rng(44)
+    spectra = np.array([0, 1, 100, 255])
+    bidx = np.concatenate([rng.choice(spectra, 1200), rng.choice(spectra, 400)])
+    nidx = np.concatenate([rng.integers(0, N, 1200), rng.integers(0, N // 64, 400)])
+    x_rows = d_x[spectra].cpu().numpy()
+    remap = {int(b): i for i, b in enumerate(spectra)}
+    tb, tn = torch.as_tensor(bidx, device="cuda"), torch.as_tensor(nidx, device="cuda")
+    for variant in VARIANTS:
+        plan = hs.hs_plan_create_ex(N, B, Hmax, variant, "reduced", "all", "c2")
+        _, vmax, amax = plan.run(d_x)
+        plan.device_status()
+        h, _ = ext.points_all(x_rows, Hmax, variant, np.array([remap[int(b)] for b in bidx]), nidx)
+        best, second, gap, m = argmax_from_levels(h)
+        check_sums(vmax[tb, tn].cpu().numpy(), m, f"all-H bench shape {variant} max")
+        check_argmax(amax[tb, tn].cpu().numpy(), best, second, gap, m, f"all-H bench shape {variant} argmax")
+        assert bool((vmax >= d_x).all()) and int(amax.max()) <= Hmax - 1
+
+
+# ------------------------------------------------------------------------------------------ two-dimensional sum
+@pytest.mark.parametrize("variant", ["standard", "freqbin"])
+def test_2d_whole_batch(hs, ext, variant):
+    rng = np.random.default_rng(51)
+    for N, Z, B, Hmax in ((8, 1, 2, 32), (100, 3, 2, 32), (4100, 9, 2, 32), (1000, 41, 1, 8), (2052, 5, 3, 2), (20000, 7, 1, 16)):
+        x = (rng.standard_exponential((B, Z, N)) - 1).astype(np.float32)
+        x[0, Z // 2, N // 3] += 30.0
+        d_x = torch.from_numpy(x).cuda()
+        for out_mode in ("both", "reduced", "full"):
+            plan = hs.hs_plan_create_2d(N, Z, B, Hmax, variant, out_mode)
+            assert (plan.algo == hs.HS_ALGO_GENERAL) == (Z > 1)        # a one-row plane is the 1-D problem
+            got = plan.run(d_x if Z > 1 else d_x.view(B, N))
+            got = tuple(None if t is None else (t if Z > 1 else t.unsqueeze(-2)) for t in got)
+            plan.device_status()
+            ref = ext.harmonic_sum_2d(x, Hmax, variant)
+            compare(plan, got, ref, f"2-D {variant}/{out_mode}/N={N}/Z={Z}/Hmax={Hmax}", x)
+
+
+def test_2d_recovers_an_integer_harmonic_track_and_matches_1d_on_the_zero_drift_row(hs):
+    Z, N, r0, z0, Zc = 129, 8192, 100, -2, 64
+    amp = (5.0 * 0.9 ** np.arange(32) + 0.25).astype(np.float32)
+    plane = np.zeros((1, Z, N), np.float32)
+    for k in range(1, 33):
+        plane[0, k * z0 + Zc, k * r0] = amp[k - 1]
+    rng = np.random.default_rng(52)
+    plane[0, Zc] = (rng.standard_exponential(N) - 1).astype(np.float32)           # noise on the zero-drift row only
+    d = torch.from_numpy(plane).cuda()
+    std, _, _ = hs.hs_plan_create_2d(N, Z, 1, 32, "standard", "full").run(d)
+    fb, _, _ = hs.hs_plan_create_2d(N, Z, 1, 32, "freqbin", "full").run(d)
+    for l, H in enumerate((1, 2, 4, 8, 16, 32)):
+        want = float(np.cumsum(amp.astype(np.float64))[H - 1]) / np.sqrt(H)
+        assert float(std[0, l, H * z0 + Zc, H * r0]) == pytest.approx(want, rel=1e-5)
+        assert float(fb[0, l, z0 + Zc, r0]) == pytest.approx(want, rel=1e-5)
+    one_d, _, _ = hs.hs_plan_create(N, 1, 32, "standard", "full").run(d[:, Zc].contiguous())
+    assert torch.equal(std[0, :, Zc], one_d[0])                                    # z = 0: the 1-D kernels' result, bit for bit
+
+
+def test_2d_sampled_at_bench_size(hs, ext):
+    """The shape bench.py --workload plane times: 8 planes of 129 drifts x 2^18 bins, reduced output."""
+    B, Z, N = 8, 129, 1 << 18
+    d_x = W.exp_noise_torch(B * Z, N, 8, "cuda").view(B, Z, N)
+    rng = np.random.default_rng(53)
+    planes = [0, 7]
+    x_rows = d_x[planes].cpu().numpy()
+    P = 1500
+    pb, pz, pn = rng.integers(0, 2, P), rng.integers(0, Z, P), rng.integers(0, N, P)
+    for variant in ("standard", "freqbin"):
+        plan = hs.hs_plan_create_2d(N, Z, B, 32, variant, "reduced")
+        _, vmax, amax = plan.run(d_x)
+        plan.device_status()
+        h = np.array([[ext.partial_sum_2d(x_rows[b], n, z, H, variant) / np.sqrt(H) for H in (1, 2, 4, 8, 16, 32)]
+                      for b, z, n in zip(pb, pz, pn)])
+        best, second, gap, m = argmax_from_levels(h)
+        tb = torch.as_tensor(np.array(planes)[pb], device="cuda")
+        tz, tn = torch.as_tensor(pz, device="cuda"), torch.as_tensor(pn, device="cuda")
+        check_sums(vmax[tb, tz, tn].cpu().numpy(), m, f"2-D bench shape {variant} max")
+        check_argmax(amax[tb, tz, tn].cpu().numpy(), best, second, gap, m, f"2-D bench shape {variant} argmax")
+        assert bool((vmax >= d_x).all())
