@@ -130,6 +130,22 @@ hs_plan *hs_plan_create_2d(int64_t nbins, int64_t nz, int64_t batch, int Hmax, i
 int hs_execute(const hs_plan *plan, const float *d_x, float *d_sums, float *d_max, uint8_t *d_argmax,
                void *stream);
 
+/*
+ * hs_execute_complex — the path with the step BEFORE it in the pipeline fused in (the series are "transformed
+ * using an FFT into frequency space.  Then the harmonic sum is applied"): instead of a normalised
+ * power spectrum the input is the complex Fourier series itself, d_F [batch][nbins][2] float32 (re, im interleaved, DEVICE,
+ * 16-byte aligned, read-only), and every kernel forms
+ *     x(k) = (re_k^2 + im_k^2) * scale - 1          fp32, each operation rounded separately (no fused multiply-add)
+ * while it reads, so that x is never written to (or re-read from) HBM.  Outputs, NULL rules, workspace rule and
+ * asynchrony as hs_execute; results are those of hs_execute on that x (bit for bit in h_1 = x).
+ * Kernels: the gathers (eqs. 3-4), the interleaved ring's copy items (eq. 3), eq. 2's grouped kernel (phase A forms x while
+ * filling shared memory) and the direct family; plans whose tuned kernel stages x with the TMA copy engine (eq. 1; eq. 2 on
+ * spectra too long for the grouped kernel) run the direct family here.  Plans of hs_plan_create_ex with non-default
+ * options and of hs_plan_create_2d: HS_ERR_INVALID_ARG.
+ */
+int hs_execute_complex(const hs_plan *plan, const float *d_F, float scale, float *d_sums, float *d_max,
+                       uint8_t *d_argmax, void *stream);
+
 /* hs_destroy — free the plan (host memory, and the staging streams if any).  NULL is a no-op returning HS_OK. */
 int hs_destroy(hs_plan *plan);
 

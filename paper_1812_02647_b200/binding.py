@@ -38,6 +38,7 @@ _SIGS = {
     "hs_plan_create_ex": ([_i64, _i64, _int, _int, _int, _int, _int], _p),
     "hs_plan_create_2d": ([_i64, _i64, _i64, _int, _int, _int], _p),
     "hs_execute": ([_p, _p, _p, _p, _p, _p], _int),
+    "hs_execute_complex": ([_p, _p, ctypes.c_float, _p, _p, _p, _p], _int),
     "hs_destroy": ([_p], _int),
     "hs_last_error": ([], _int),
     "hs_error_string": ([_int], ctypes.c_char_p),
@@ -161,6 +162,25 @@ class Plan:
     def hs_execute(self, d_x, d_sums=None, d_max=None, d_argmax=None, stream=None):
         _check(lib.hs_execute(self.handle, _ptr(d_x), _ptr(d_sums), _ptr(d_max), _ptr(d_argmax), _stream(stream)),
                "hs_execute")
+
+    def hs_execute_complex(self, d_F, scale, d_sums=None, d_max=None, d_argmax=None, stream=None):
+        """d_F: complex64 (or float32 [..., 2]) CUDA tensor [batch][nbins]; x = |F|^2 * scale - 1 is formed inside the kernels."""
+        _check(lib.hs_execute_complex(self.handle, _ptr(d_F), ctypes.c_float(scale), _ptr(d_sums), _ptr(d_max),
+                                      _ptr(d_argmax), _stream(stream)), "hs_execute_complex")
+
+    def run_complex(self, d_F, scale, stream=None):
+        """Allocate the outputs, execute on the complex series, return (sums, max, argmax)."""
+        import torch
+        assert d_F.is_cuda and d_F.is_contiguous() and tuple(d_F.shape[:2]) == (self.batch, self.nbins)
+        sums = vmax = amax = None
+        if self.out_mode & HS_OUT_FULL:
+            sums = torch.empty((self.batch, self.levels, self.nbins), dtype=torch.float32, device=d_F.device)
+        if self.out_mode & HS_OUT_REDUCED:
+            vmax = torch.empty((self.batch, self.nbins), dtype=torch.float32, device=d_F.device)
+            amax = torch.empty((self.batch, self.nbins), dtype=torch.uint8, device=d_F.device)
+        self.ensure_workspace(d_F.device)
+        self.hs_execute_complex(d_F, scale, sums, vmax, amax, stream)
+        return sums, vmax, amax
 
     def host_staging_bytes(self, slab_spectra: int) -> int:
         return lib.hs_plan_host_staging_bytes(self.handle, int(slab_spectra))

@@ -75,7 +75,7 @@ int check_buffers(const hs_plan *p, const void *x, const void *sums, const void 
 
 int launch_family(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
-    if (p->algo == HS_ALGO_TILED) return hs_launch_tiled(p, buf, batch, ws, stream);
+    if (p->algo == HS_ALGO_TILED && (!buf.cplx || hs_tiled_supports_complex(p))) return hs_launch_tiled(p, buf, batch, ws, stream);
     if (p->algo == HS_ALGO_GENERAL) return hs_launch_general(p, buf, batch, ws, stream);
     return hs_launch_direct(p, buf, batch, ws, stream);
 }
@@ -281,7 +281,22 @@ int hs_execute(const hs_plan *p, const float *d_x, float *d_sums, float *d_max, 
     if (hs_plan_workspace_bytes(p) > 0 && (!p->ws || p->ws_bytes < hs_plan_workspace_bytes(p))) HS_FAIL(HS_ERR_WORKSPACE);
     note_ctrl(p, p->ws, true);
     hs_buffers buf{d_x, (p->out_mode & HS_OUT_FULL) ? d_sums : nullptr, (p->out_mode & HS_OUT_REDUCED) ? d_max : nullptr,
-                   (p->out_mode & HS_OUT_REDUCED) ? d_argmax : nullptr, nullptr, {}};
+                   (p->out_mode & HS_OUT_REDUCED) ? d_argmax : nullptr, nullptr, {}, false, 0.0f};
+    return launch_family(p, buf, p->batch, p->ws, static_cast<cudaStream_t>(stream));
+}
+
+int hs_execute_complex(const hs_plan *p, const float *d_F, float scale, float *d_sums, float *d_max, uint8_t *d_argmax,
+                       void *stream)
+{
+    int rc = check_buffers(p, d_F, d_sums, d_max, d_argmax);
+    if (rc != HS_OK) return rc;
+    if (is_general(p) || !(scale == scale)) HS_FAIL(HS_ERR_INVALID_ARG);
+    if ((rc = check_device(p)) != HS_OK) return rc;
+    const bool tiled = p->algo == HS_ALGO_TILED && hs_tiled_supports_complex(p);
+    if (tiled && hs_plan_workspace_bytes(p) > 0 && (!p->ws || p->ws_bytes < hs_plan_workspace_bytes(p))) HS_FAIL(HS_ERR_WORKSPACE);
+    note_ctrl(p, tiled ? p->ws : nullptr, true);
+    hs_buffers buf{d_F, (p->out_mode & HS_OUT_FULL) ? d_sums : nullptr, (p->out_mode & HS_OUT_REDUCED) ? d_max : nullptr,
+                   (p->out_mode & HS_OUT_REDUCED) ? d_argmax : nullptr, nullptr, {}, true, scale};
     return launch_family(p, buf, p->batch, p->ws, static_cast<cudaStream_t>(stream));
 }
 
@@ -297,7 +312,7 @@ int hs_execute_candidates(const hs_plan *p, const float *d_x, float threshold, h
     note_ctrl(p, p->ws, true);
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     HS_CUDA_OK(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s));
-    hs_buffers buf{d_x, nullptr, nullptr, nullptr, nullptr, {}};
+    hs_buffers buf{d_x, nullptr, nullptr, nullptr, nullptr, {}, false, 0.0f};
     // a kernel tests `cand` to choose between appending and storing: with no room at all it still has to count
     static hs_candidate *const kNowhere = reinterpret_cast<hs_candidate *>(16);
     buf.sink.cand = capacity > 0 ? d_cand : kNowhere;
@@ -318,7 +333,7 @@ int hs_debug_greedy_paths(const hs_plan *p, const float *d_x, uint8_t *d_j, void
     if (hs_plan_workspace_bytes(p) > 0 && (!p->ws || p->ws_bytes < hs_plan_workspace_bytes(p))) HS_FAIL(HS_ERR_WORKSPACE);
     note_ctrl(p, p->ws, true);
     // the plan's own kernel family in its own launch configuration, writing j instead of the outputs
-    hs_buffers buf{d_x, nullptr, nullptr, nullptr, d_j, {}};
+    hs_buffers buf{d_x, nullptr, nullptr, nullptr, d_j, {}, false, 0.0f};
     return launch_family(p, buf, p->batch, p->ws, static_cast<cudaStream_t>(stream));
 }
 
@@ -387,7 +402,7 @@ int hs_execute_host(hs_plan *p, const float *h_x, float *h_sums, float *h_max, u
         void *dws = lay.ws ? base + lay.x + lay.sums + lay.vmax + lay.amax : nullptr;
         cudaStream_t s = p->lane_stream[lane];
         HS_CUDA_OK(cudaMemcpyAsync(dx, h_x + (size_t)b0 * N, bins * 4, cudaMemcpyHostToDevice, s));
-        hs_buffers buf{dx, dsums, dmax, damax, nullptr, {}};
+        hs_buffers buf{dx, dsums, dmax, damax, nullptr, {}, false, 0.0f};
         note_ctrl(p, dws, false);
         const int rc = launch_family(p, buf, nb, dws, s);
         if (rc != HS_OK) return rc;

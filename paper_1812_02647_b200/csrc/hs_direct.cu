@@ -7,25 +7,24 @@ namespace {
 
 constexpr int kThreads = 256;
 
-__device__ __forceinline__ float ldz(const float *__restrict__ x, int k, int N)
-{
-    return k < N ? __ldg(x + k) : 0.0f;  // zero padding, C5
-}
-
-template <int VARIANT, int L, int OUT, bool JDBG>
+// CPLX (hs_execute_complex): x holds the complex Fourier series, every read forms the normalised power on the fly.
+template <int VARIANT, int L, int OUT, bool JDBG, bool CPLX>
 __global__ void __launch_bounds__(kThreads)
 hs_direct_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
-                 uint8_t *__restrict__ amax, uint8_t *__restrict__ jdbg, int N, int tiles_per_spectrum, hs_cand_sink sink)
+                 uint8_t *__restrict__ amax, uint8_t *__restrict__ jdbg, int N, int tiles_per_spectrum, hs_cand_sink sink,
+                 float scale)
 {
     const int64_t b = blockIdx.x / tiles_per_spectrum;
     const int n = (blockIdx.x % tiles_per_spectrum) * kThreads + threadIdx.x;
     if (n >= N) return;
-    const float *__restrict__ xb = x + b * (int64_t)N;
+    const float *__restrict__ xb = x + b * (int64_t)N * (CPLX ? 2 : 1);
+    auto ld = [&](int k) { return hs_ldx<CPLX>(xb, k, scale); };
+    auto ldz = [&](const float *, int k, int) { return k < N ? hs_ldx<CPLX>(xb, k, scale) : 0.0f; };   // zero padding, C5
     float *plane0 = (OUT & HS_OUT_FULL) ? sums + (b * L) * (int64_t)N + n : nullptr;
     uint8_t *jplane0 = JDBG ? jdbg + (b * L) * (int64_t)N + n : nullptr;
     hs_emit<OUT> e;
 
-    float S = __ldg(xb + n);
+    float S = ld(n);
     e.level(0, S, plane0, N);
     if (JDBG) jplane0[0] = 0;
 
@@ -36,7 +35,7 @@ hs_direct_kernel(const float *__restrict__ x, float *__restrict__ sums, float *_
         for (int l = 1; l < L; l++) {
             const int H = 1 << l;
 #pragma unroll
-            for (int i = 1; i < H; i += 2) S += __ldg(xb + ((n * i + (H >> 1)) >> l));
+            for (int i = 1; i < H; i += 2) S += ld((n * i + (H >> 1)) >> l);
             e.level(l, S, plane0, N);
         }
     } else if (VARIANT == HS_FREQBIN) {
@@ -83,8 +82,8 @@ hs_direct_kernel(const float *__restrict__ x, float *__restrict__ sums, float *_
     }
 }
 
-template <int VARIANT, int L, int OUT, bool JDBG>
-int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+template <int VARIANT, int L, int OUT, bool JDBG, bool CPLX>
+int launch_c(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     const int N = (int)p->nbins;
     const int tiles = (N + kThreads - 1) / kThreads;
@@ -94,12 +93,19 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t 
         const int64_t off = b0 * (int64_t)N;
         hs_cand_sink sink = buf.sink;
         sink.b0 += (int)b0;
-        hs_direct_kernel<VARIANT, L, OUT, JDBG><<<(unsigned)(nb * tiles), kThreads, 0, stream>>>(
-            buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
-            buf.amax ? buf.amax + off : nullptr, buf.jdbg ? buf.jdbg + off * L : nullptr, N, tiles, sink);
+        hs_direct_kernel<VARIANT, L, OUT, JDBG, CPLX><<<(unsigned)(nb * tiles), kThreads, 0, stream>>>(
+            buf.x + off * (CPLX ? 2 : 1), buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
+            buf.amax ? buf.amax + off : nullptr, buf.jdbg ? buf.jdbg + off * L : nullptr, N, tiles, sink, buf.scale);
         HS_CUDA_OK(cudaGetLastError());
     }
     return HS_OK;
+}
+
+template <int VARIANT, int L, int OUT, bool JDBG>
+int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+{
+    if (buf.cplx) return launch_c<VARIANT, L, OUT, JDBG, true>(p, buf, batch, stream);
+    return launch_c<VARIANT, L, OUT, JDBG, false>(p, buf, batch, stream);
 }
 
 template <int VARIANT, int L>

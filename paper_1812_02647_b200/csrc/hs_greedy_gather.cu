@@ -64,10 +64,11 @@ __device__ __forceinline__ float max_window_rt(const float *__restrict__ w, int 
 // spectra in flight per CTA row would not fit L2): the Q chains are the bins n, n + 128, .., n + 128 (Q - 1) of ONE
 // spectrum; the warp-uniform bounds then span the CTA's Q blocks (safe: in range for the last block; any: for the first).
 // JDBG (hs_debug_greedy_paths, eq. 4 only, OUT = 0): the drift j after each level goes to jdbg[b][l][n] instead of the outputs.
-template <int VARIANT, int L, int OUT, int Q, bool SAME, bool JDBG = false>
+// CPLX (hs_execute_complex): x holds the complex Fourier series, every read forms the normalised power on the fly.
+template <int VARIANT, int L, int OUT, int Q, bool SAME, bool JDBG = false, bool CPLX = false>
 __global__ void __launch_bounds__(kThreads, Q >= 8 ? 8 : 12)
 hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
-                        uint8_t *__restrict__ amax, uint8_t *__restrict__ jdbg, int N, int batch, hs_cand_sink sink)
+                        uint8_t *__restrict__ amax, uint8_t *__restrict__ jdbg, int N, int batch, hs_cand_sink sink, float scale)
 {
     const int n = blockIdx.x * (SAME ? kThreads * Q : kThreads) + threadIdx.x;
     const int n_lo = n & ~31;                      // first bin of this warp (of its first block)
@@ -95,8 +96,8 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
 #pragma unroll
         for (int q = 0; q < Q; q++) {
             live[q] = valid[SAME ? q : 0] && b0 + (SAME ? 0 : q) < batch;
-            xb[q] = x + (int64_t)min(b0 + (SAME ? 0 : q), batch - 1) * N;   // spectra past the batch shadow the last one
-            S[q] = __ldg(xb[q] + nn[SAME ? q : 0]);
+            xb[q] = x + (int64_t)min(b0 + (SAME ? 0 : q), batch - 1) * N * (CPLX ? 2 : 1);   // spectra past the batch shadow the last one
+            S[q] = hs_ldx<CPLX>(xb[q], nn[SAME ? q : 0], scale);
             j[q] = 0;
         }
         auto emit = [&](int l) {
@@ -115,19 +116,19 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
             for (int q = 0; q < Q; q++) {
                 const int base = bases[SAME ? q : 0];
                 if (VARIANT == HS_FREQBIN) {        // eq. 3: x~(i n)
-                    S[q] += (safe || base < N) ? __ldg(xb[q] + base) : 0.0f;
+                    S[q] += (safe || base < N) ? hs_ldx<CPLX>(xb[q], base, scale) : 0.0f;
                 } else if (VARIANT == HS_MAX) {     // eq. 2 (Hmax <= 8): maximum of the aligned block x~[i n .. i n + i - 1]
-                    if (safe) {
+                    if (safe && !CPLX) {
                         S[q] += max_window_rt(xb[q] + base, i);
                     } else {
-                        float m = base < N ? __ldg(xb[q] + base) : 0.0f;
-                        for (int t = 1; t < i; t++) m = fmaxf(m, base + t < N ? __ldg(xb[q] + base + t) : 0.0f);
+                        float m = base < N ? hs_ldx<CPLX>(xb[q], base, scale) : 0.0f;
+                        for (int t = 1; t < i; t++) m = fmaxf(m, base + t < N ? hs_ldx<CPLX>(xb[q], base + t, scale) : 0.0f);
                         S[q] += m;
                     }
                 } else {                            // eq. 4: max of the bin under the drift and its right neighbour
                     const int k = base + j[q];
-                    const float lft = (safe || k < N) ? __ldg(xb[q] + k) : 0.0f;
-                    const float rgt = (safe || k + 1 < N) ? __ldg(xb[q] + k + 1) : 0.0f;
+                    const float lft = (safe || k < N) ? hs_ldx<CPLX>(xb[q], k, scale) : 0.0f;
+                    const float rgt = (safe || k + 1 < N) ? hs_ldx<CPLX>(xb[q], k + 1, scale) : 0.0f;
                     const bool right = rgt > lft;   // strictly greater (C4)
                     S[q] += right ? rgt : lft;
                     j[q] += right ? 1 : 0;
@@ -181,8 +182,8 @@ hs_greedy_gather_kernel(const float *__restrict__ x, float *__restrict__ sums, f
     }
 }
 
-template <int VARIANT, int L, int OUT, int Q, bool SAME = false, bool JDBG = false>
-int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+template <int VARIANT, int L, int OUT, int Q, bool SAME, bool JDBG, bool CPLX>
+int launch_qc(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
     const int N = (int)p->nbins;
     const int per_cta = SAME ? kThreads * Q : kThreads;
@@ -195,12 +196,21 @@ int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_
         const dim3 grid((unsigned)tiles, (unsigned)(gy < kGridY ? gy : kGridY), 1);
         hs_cand_sink sink = buf.sink;
         sink.b0 += (int)b0;
-        hs_greedy_gather_kernel<VARIANT, L, OUT, Q, SAME, JDBG><<<grid, kThreads, 0, stream>>>(
-            buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
-            buf.amax ? buf.amax + off : nullptr, buf.jdbg ? buf.jdbg + off * L : nullptr, N, (int)nb, sink);
+        hs_greedy_gather_kernel<VARIANT, L, OUT, Q, SAME, JDBG, CPLX><<<grid, kThreads, 0, stream>>>(
+            buf.x + off * (CPLX ? 2 : 1), buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
+            buf.amax ? buf.amax + off : nullptr, buf.jdbg ? buf.jdbg + off * L : nullptr, N, (int)nb, sink, buf.scale);
         HS_CUDA_OK(cudaGetLastError());
     }
     return HS_OK;
+}
+
+template <int VARIANT, int L, int OUT, int Q, bool SAME = false, bool JDBG = false>
+int launch_q(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
+{
+    if constexpr (!JDBG) {
+        if (buf.cplx) return launch_qc<VARIANT, L, OUT, Q, SAME, false, true>(p, buf, batch, stream);
+    }
+    return launch_qc<VARIANT, L, OUT, Q, SAME, JDBG, false>(p, buf, batch, stream);
 }
 
 // Spectra side by side per thread: 8 while 8 spectra (and what is in flight around them) stay in L2; longer spectra run

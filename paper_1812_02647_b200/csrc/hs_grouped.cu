@@ -89,6 +89,7 @@ struct gr_params {
     int n_split;     // multiple of kChunk, >= N/2: the outputs of bins n >= n_split are emitted by phase A
     hs_cand_sink sink;
     unsigned spin_limit;
+    float scale;     // CPLX (hs_execute_complex): x holds (re, im) pairs, x(k) = hs_power(F_k, scale)
 };
 
 constexpr int chain_len(int j, int hmax)  // K_j: largest power of two with j*K <= hmax
@@ -435,19 +436,19 @@ __device__ __forceinline__ void phaseA_chunk(const gr_params &p, const gr_smem &
 // The loads of a level are issued in batches of up to 8 float4 before they are consumed (memory-level parallelism).
 // Terms of harmonic I for the outputs n .. n + 3 straight from the spectrum: the window x[I n .. I n + 4 I) as I aligned
 // float4 loads (`whole`: warp-uniform, every element of the warp's windows in range), else element-wise with zero padding.
-template <int VARIANT, int I>
-__device__ __forceinline__ void add_from_x(float4 &S, const float *__restrict__ xrow, int n, int N, bool whole)
+template <int VARIANT, int I, bool CPLX>
+__device__ __forceinline__ void add_from_x(float4 &S, const float *__restrict__ xrow, int n, int N, bool whole, float scale)
 {
     float v[4 * I];
     if (whole) {
 #pragma unroll
         for (int q = 0; q < I; q++) {
-            const float4 t = __ldg(reinterpret_cast<const float4 *>(xrow + I * n) + q);
+            const float4 t = hs_ldx4<CPLX>(xrow, I * n + 4 * q, scale);
             v[4 * q] = t.x, v[4 * q + 1] = t.y, v[4 * q + 2] = t.z, v[4 * q + 3] = t.w;
         }
     } else {
 #pragma unroll
-        for (int k = 0; k < 4 * I; k++) v[k] = I * n + k < N ? __ldg(xrow + I * n + k) : 0.0f;   // zero padding (C5)
+        for (int k = 0; k < 4 * I; k++) v[k] = I * n + k < N ? hs_ldx<CPLX>(xrow, I * n + k, scale) : 0.0f;   // zero padding (C5)
     }
     float t[4];
 #pragma unroll
@@ -464,13 +465,14 @@ __device__ __forceinline__ void add_from_x(float4 &S, const float *__restrict__ 
     S.w += t[3];
 }
 
-template <int L, int OUT, int VARIANT = HS_MAX, int HYB = 0>
+template <int L, int OUT, int VARIANT = HS_MAX, int HYB = 0, bool CPLX = false>
 __device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__restrict__ Ab, int64_t row, int n_first)
 {
     const int N = p.N;
     const int n = n_first + 4 * (threadIdx.x & 31);
     const bool live = n < N;                                       // (N % 4 == 0: a float4 is wholly inside or outside)
-    float4 S = live ? __ldg(reinterpret_cast<const float4 *>(p.x + row + n)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float *__restrict__ xrow = p.x + row * (CPLX ? 2 : 1);
+    float4 S = live ? hs_ldx4<CPLX>(xrow, n, p.scale) : make_float4(0.f, 0.f, 0.f, 0.f);
     hs_emit<OUT> e0, e1, e2, e3;
     const float *__restrict__ An = Ab + ((unsigned)n);       // A_i[n] = An[off_i]
     auto emit = [&](int l) {
@@ -492,12 +494,11 @@ __device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__r
         const int lo = (1 << (l - 1)) + 1, hi = 1 << l;
         if ((int64_t)lo * n_first < N) {                           // warp-uniform: the level has a harmonic in range
             if (HYB == 2 && l <= 2) {                              // sizes 2, 3, 4 are not kept: straight from the spectrum
-                const float *__restrict__ xrow = p.x + row;
                 if (l == 1) {
-                    add_from_x<VARIANT, 2>(S, xrow, n, N, 2 * (n_first + kTileB) <= N);
+                    add_from_x<VARIANT, 2, CPLX>(S, xrow, n, N, 2 * (n_first + kTileB) <= N, p.scale);
                 } else {
-                    add_from_x<VARIANT, 3>(S, xrow, n, N, 3 * (n_first + kTileB) <= N);
-                    add_from_x<VARIANT, 4>(S, xrow, n, N, 4 * (n_first + kTileB) <= N);
+                    add_from_x<VARIANT, 3, CPLX>(S, xrow, n, N, 3 * (n_first + kTileB) <= N, p.scale);
+                    add_from_x<VARIANT, 4, CPLX>(S, xrow, n, N, 4 * (n_first + kTileB) <= N, p.scale);
                 }
             } else if ((int64_t)hi * (n_first + kTileB) <= N) {    // warp-uniform: every element of the level in range
 #pragma unroll
@@ -559,7 +560,10 @@ struct gr_pos {
     int b, c;  // spectrum, chunk
 };
 
-template <int VARIANT, int HMAX, int OUT, int HYB>
+// CPLX (hs_execute_complex): x holds the complex Fourier series.  Phase A loads the chunk with ordinary vector loads and
+// forms the normalised power while writing it to shared memory (no TMA: the copy engine cannot compute); phase B forms
+// the few values it reads from the spectrum on the fly.  x itself is never written to global memory.
+template <int VARIANT, int HMAX, int OUT, int HYB, bool CPLX = false>
 __global__ void __launch_bounds__(kThreads, 4)
 gr_kernel(const __grid_constant__ gr_params p)
 {
@@ -590,6 +594,7 @@ gr_kernel(const __grid_constant__ gr_params p)
 
     // thread 0: start the TMA bulk copy of chunk `at` into buffer `buf` (the part that lies inside the spectrum)
     auto issue = [&](gr_pos at, int buf) {
+        if (CPLX) return;                                                 // (loaded by all threads in the chunk loop)
         const int k0 = at.c * kChunk;
         const int words = min(kChunk + kHalo, N - k0);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // the buffer was last written by ordinary stores
@@ -629,10 +634,16 @@ gr_kernel(const __grid_constant__ gr_params p)
                 const int lenK = (p.lay.len[i] + K - 1) / K * K;          // whole super-blocks that start in the spectrum
                 s_bounds[i] = make_int2(first, min(last, lenK));
             }
-            hsptx::mbar_wait(&bar[buf], (parity >> buf) & 1u);
-            parity ^= 1u << buf;
             sm.raw = dyn + buf * kRaw;
             const int valid = min(kChunk + kHalo, N - k0);                // words the copy delivered (multiple of 4)
+            if (CPLX) {
+                const float *__restrict__ frow = p.x + ((int64_t)b * N + k0) * 2;
+                for (int w = 4 * threadIdx.x; w < valid; w += 4 * kThreads)
+                    *reinterpret_cast<float4 *>(sm.raw + w) = hs_ldx4<true>(frow, w, p.scale);
+            } else {
+                hsptx::mbar_wait(&bar[buf], (parity >> buf) & 1u);
+                parity ^= 1u << buf;
+            }
             for (int w = valid + threadIdx.x; w < kRaw; w += kThreads) sm.raw[w] = 0.0f;   // zero padding (C5)
             __syncthreads();
             phaseA_chunk<VARIANT, HMAX, HYB>(p, sm, Ab, k0);
@@ -656,7 +667,7 @@ gr_kernel(const __grid_constant__ gr_params p)
             j = __shfl_sync(0xffffffffu, j, 0);
             const int tile = rank + p.GS * j;
             if (tile >= p.ntiles) break;
-            phaseB_tile<L, OUT, VARIANT, HYB>(p, Ab, row, tile * kTileB);
+            phaseB_tile<L, OUT, VARIANT, HYB, CPLX>(p, Ab, row, tile * kTileB);
         }
         __syncthreads();                                                  // every load of the slot has returned
         if (threadIdx.x == 0) red_release_add(cntB, 1);
@@ -710,8 +721,8 @@ size_t smem_bytes(int variant, int Hmax)
     return (size_t)((tabs ? 1 : 2) * kRaw + tabs * kTab) * sizeof(float);
 }
 
-template <int VARIANT, int HMAX, int OUT, int HYB>
-int launch_hyb(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+template <int VARIANT, int HMAX, int OUT, int HYB, bool CPLX>
+int launch_hyb_c(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
     const gr_sched s = make_sched(p, batch);
     gr_params prm{};
@@ -731,7 +742,8 @@ int launch_hyb(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws,
     prm.ntiles = s.ntiles;
     prm.n_split = s.n_split;
     prm.spin_limit = hs_spin_limit();
-    auto kern = gr_kernel<VARIANT, HMAX, OUT, HYB>;
+    prm.scale = buf.scale;
+    auto kern = gr_kernel<VARIANT, HMAX, OUT, HYB, CPLX>;
     const size_t smem = smem_bytes(VARIANT, HMAX);
     // (function attributes are per device: set on every launch rather than once per process)
     HS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -744,6 +756,16 @@ int launch_hyb(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws,
     HS_CUDA_OK(cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(kern), dim3((unsigned)(s.groups * s.GS)),
                                            dim3(kThreads), args, smem, stream));
     return HS_OK;
+}
+
+template <int VARIANT, int HMAX, int OUT, int HYB>
+int launch_hyb(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    if constexpr (VARIANT == HS_MAX && HMAX >= 8) {                      // (the complex front end: where this kernel is a default)
+        if (buf.cplx) return launch_hyb_c<VARIANT, HMAX, OUT, HYB, true>(p, buf, batch, ws, stream);
+    }
+    if (buf.cplx) HS_FAIL(HS_ERR_INVALID_ARG);
+    return launch_hyb_c<VARIANT, HMAX, OUT, HYB, false>(p, buf, batch, ws, stream);
 }
 
 template <int VARIANT, int HMAX, int OUT>

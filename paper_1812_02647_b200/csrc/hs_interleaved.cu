@@ -64,6 +64,7 @@ struct il_params {
     unsigned spin_limit;
     int64_t slot_words;
     int N, B, groups, R;
+    float scale;        // CPLX (hs_execute_complex): x holds (re, im) pairs, the copy items form x = |F|^2 scale - 1
     hs_cand_sink sink;
     int nT, nG;         // items per group
     int nHeavy;         // the first nHeavy G items are single tiles (bins below ~N/8: 8 to 32 harmonics per bin)
@@ -74,7 +75,6 @@ struct il_params {
 // Ring data: ordinary weak loads (L1-allocating).  Coherent here because a CTA's first read of a group follows its own
 // acquire of the group's counter (LDG.E.STRONG.GPU + CCTL.IVALL: the SM's L1 is invalidated) and a __syncthreads.
 __device__ __forceinline__ float4 ld_ring(const float4 *p) { return *p; }
-__device__ __forceinline__ float ld_ring(const float *p) { return *p; }
 
 __device__ __forceinline__ float4 ld_stream(const float4 *p)   // read-once input: evict-first in L1 and L2
 {
@@ -84,7 +84,7 @@ __device__ __forceinline__ float4 ld_stream(const float4 *p)   // read-once inpu
 }
 // ------------------------------------------------------------------------------------------------ T item
 // xT[k][g] = x[b0 + g][k] for g < nb, 0 for nb <= g < G, k in [k0, k0 + 512) below N; outputs of the bins >= n_split.
-template <int L, int OUT, class F>
+template <int L, int OUT, bool CPLX, class F>
 __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int grp, int k0, float *__restrict__ xT, F &redraw)
 {
     const int N = p.N;
@@ -101,7 +101,16 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
         for (int q = 0; q < Q; q++) {
             const int k = k0 + 4 * (lane + 32 * q);
             v[s][q] = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (g < nb && k < N) v[s][q] = ld_stream(reinterpret_cast<const float4 *>(p.x + (b0 + g) * N + k));
+            if (g < nb && k < N) {
+                if (CPLX) {                               // the fused front end: x is formed here and never written to HBM
+                    const float4 *f = reinterpret_cast<const float4 *>(p.x + ((b0 + g) * N + k) * 2);
+                    const float4 a = ld_stream(f), c = ld_stream(f + 1);
+                    v[s][q] = make_float4(hs_power(a.x, a.y, p.scale), hs_power(a.z, a.w, p.scale),
+                                          hs_power(c.x, c.y, p.scale), hs_power(c.z, c.w, p.scale));
+                } else {
+                    v[s][q] = ld_stream(reinterpret_cast<const float4 *>(p.x + (b0 + g) * N + k));
+                }
+            }
         }
     }
     redraw();                                           // (thread 0: the next item, while the loads are in flight)
@@ -320,7 +329,7 @@ using hssync::kNoTicket;
 using il_tickets = hssync::tickets;
 constexpr int kItemG = 1 << 30;
 
-template <int L, int OUT>
+template <int L, int OUT, bool CPLX>
 __global__ void __launch_bounds__(kThreads, 2)
 il_persistent_kernel(const __grid_constant__ il_params p)
 {
@@ -353,7 +362,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
         if (!(item & kItemG)) {                                         // ---- T item
             const int s = item / p.nT, idx = item - s * p.nT;
             float *xT = p.xT + (int64_t)(s % p.R) * p.slot_words;
-            copy_item<L, OUT>(p, tile, s, idx * kTBins, xT, redraw);
+            copy_item<L, OUT, CPLX>(p, tile, s, idx * kTBins, xT, redraw);
             __syncthreads();                                            // all stores of the CTA are ordered before ...
             if (threadIdx.x == 0) {
                 __threadfence();                                        // ... thread 0's release at gpu scope
@@ -429,8 +438,8 @@ il_sched make_sched(const hs_plan *p, int64_t batch)
 
 size_t ctrl_bytes(int groups) { return ((size_t)(16 + 2 * (size_t)groups) * sizeof(int) + 255) / 256 * 256; }
 
-template <int L, int OUT>
-int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+template <int L, int OUT, bool CPLX>
+int launch_c(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
     const il_sched s = make_sched(p, batch);
     il_params prm{};
@@ -446,13 +455,14 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     prm.B = (int)batch;
     prm.groups = s.groups;
     prm.R = s.R;
+    prm.scale = buf.scale;
     prm.spin_limit = hs_spin_limit();
     prm.nT = s.nT;
     prm.nG = s.nG;
     prm.nHeavy = s.nHeavy;
     prm.gsub = s.gsub;
     prm.n_split = s.n_split;
-    auto kern = il_persistent_kernel<L, OUT>;
+    auto kern = il_persistent_kernel<L, OUT, CPLX>;
     int occ = 0;                                                        // (per device: asked on every launch)
     HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, 0));
     const int ctas_per_sm = occ > 0 ? occ : 1;
@@ -462,6 +472,13 @@ int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cud
     kern<<<(unsigned)(total < slots ? total : slots), kThreads, 0, stream>>>(prm);
     HS_CUDA_OK(cudaGetLastError());
     return HS_OK;
+}
+
+template <int L, int OUT>
+int launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
+{
+    if (buf.cplx) return launch_c<L, OUT, true>(p, buf, batch, ws, stream);
+    return launch_c<L, OUT, false>(p, buf, batch, ws, stream);
 }
 
 template <int L>

@@ -90,12 +90,14 @@ struct hs_cand_sink {
     int b0;
 };
 struct hs_buffers {
-    const float *x;
+    const float *x;  // the spectra, or (cplx) the complex Fourier series [..][2] they are formed from on the fly
     float *sums;
     float *vmax;
     uint8_t *amax;
     uint8_t *jdbg;  // Greedy debug paths or nullptr
     hs_cand_sink sink;
+    bool cplx;      // hs_execute_complex: x holds (re, im) pairs, x(k) = hs_power(F_k, scale)
+    float scale;
 };
 int hs_launch_direct(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
 int hs_launch_general(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);   // hs_general.cu
@@ -123,7 +125,38 @@ int hs_grouped_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, vo
 int hs_grouped_launches(const hs_plan *p, int64_t batch);
 size_t hs_grouped_workspace_bytes(const hs_plan *p, int64_t batch);
 bool hs_grouped_supported(const hs_plan *p);
-bool hs_tiled_has_ctrl(const hs_plan *p);   // the resolved kernel starts its workspace with a control block
+bool hs_tiled_has_ctrl(const hs_plan *p);
+bool hs_tiled_supports_complex(const hs_plan *p);   // the resolved kernel starts its workspace with a control block
+
+// ---- fused front end (hs_execute_complex) ----------------------------------------------------
+// x(k) = (re^2 + im^2) * scale - 1, fp32, every operation rounded on its own (the _rn intrinsics are never contracted
+// into a fused multiply-add): bit-identical to oracle/hs_oracle_ext.c hsx_power_spectrum, so that the comparisons the
+// harmonic sum takes on x (Greedy's drift, the best level) are the same on both sides.
+__device__ __forceinline__ float hs_power(float re, float im, float scale)
+{
+    return __fsub_rn(__fmul_rn(__fadd_rn(__fmul_rn(re, re), __fmul_rn(im, im)), scale), 1.0f);
+}
+// element k of a spectrum whose storage starts at `row` (CPLX: `row` points at the spectrum's first (re, im) pair)
+template <bool CPLX>
+__device__ __forceinline__ float hs_ldx(const float *__restrict__ row, int k, float scale)
+{
+    if (CPLX) {
+        const float2 f = __ldg(reinterpret_cast<const float2 *>(row) + k);
+        return hs_power(f.x, f.y, scale);
+    }
+    return __ldg(row + k);
+}
+// elements k .. k + 3 (k % 4 == 0 and the row 16-byte aligned)
+template <bool CPLX>
+__device__ __forceinline__ float4 hs_ldx4(const float *__restrict__ row, int k, float scale)
+{
+    if (CPLX) {
+        const float4 a = __ldg(reinterpret_cast<const float4 *>(row) + (k >> 1));
+        const float4 b = __ldg(reinterpret_cast<const float4 *>(row) + (k >> 1) + 1);
+        return make_float4(hs_power(a.x, a.y, scale), hs_power(a.z, a.w, scale), hs_power(b.x, b.y, scale), hs_power(b.z, b.w, scale));
+    }
+    return __ldg(reinterpret_cast<const float4 *>(row + k));
+}
 
 // ---- device-side epilogue ---------------------------------------------------------------------------------------
 // c_H = fp32(1/sqrt(H)) for H = 1,2,4,8,16,32 (CONVENTIONS.md C7; "1/sqrt(H)").

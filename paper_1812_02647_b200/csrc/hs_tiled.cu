@@ -72,3 +72,13 @@ bool hs_tiled_has_ctrl(const hs_plan *p)
     if (p->variant == HS_STANDARD) return hs_standard_rb_supported(p);   // (tile counter; the error word stays zero)
     return grouped(p) || interleaved(p);
 }
+
+// hs_execute_complex: which resolved kernels form x from the complex series themselves (the others fall back to the
+// direct family, which does): the gathers, the interleaved copy items, and eq. 2's grouped kernel at Hmax >= 8.
+bool hs_tiled_supports_complex(const hs_plan *p)
+{
+    if (p->variant == HS_STANDARD) return false;                        // (both eq. 1 kernels stage x by TMA bulk copies)
+    if (p->variant == HS_MAX) return max_gather(p) || (grouped(p) && p->Hmax >= 8);
+    if (grouped(p) || two_phase(p)) return false;                       // (eq. 3 through the two-phase families: only when asked for)
+    return true;                                                        // interleaved (eq. 3) or the plain gather (eqs. 3-4)
+}

@@ -198,3 +198,84 @@ def test_2d_sampled_at_bench_size(hs, ext):
         check_sums(vmax[tb, tz, tn].cpu().numpy(), m, f"2-D bench shape {variant} max")
         check_argmax(amax[tb, tz, tn].cpu().numpy(), best, second, gap, m, f"2-D bench shape {variant} argmax")
         assert bool((vmax >= d_x).all())
+
+
+# ------------------------------------------------------------------------------------------ fused front end
+def complex_batch(B, N, seed, n_norm=312500.0):
+    """Fourier series whose normalised power is Exp(1) - 1 noise plus a few bright harmonics: F = sqrt(n/2) (g1 + i g2)."""
+    rng = np.random.default_rng(seed)
+    F = (rng.standard_normal((B, N)) + 1j * rng.standard_normal((B, N))) * np.sqrt(n_norm / 2)
+    for b in range(B):
+        m = int(rng.integers(20, max(21, N // 40)))
+        k = m * np.arange(1, 33)
+        k = k[k < N]
+        F[b, k] += np.sqrt(n_norm) * (6.0 * 0.9 ** np.arange(k.size)) * np.exp(2j * np.pi * rng.random(k.size))
+    return F.astype(np.complex64), np.float32(1.0 / n_norm)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_complex_input_whole_batch(hs, ext, oracle, variant):
+    """hs_execute_complex against the oracle composition power spectrum (fp32, step by step) -> harmonic sum, and against
+    hs_execute on the same x: the kernels that form x themselves must reproduce it bit for bit."""
+    for N, B, Hmax in ((20000, 3, 32), (1 << 15, 5, 32), (4100, 2, 8), (2052, 3, 2), (1 << 15, 17, 16)):
+        F, scale = complex_batch(B, N, 60 + Hmax)
+        x = ext.power_spectrum(F, float(scale))
+        d_F = torch.view_as_real(torch.from_numpy(F)).contiguous().cuda()
+        d_x = torch.from_numpy(x).cuda()
+        for out_mode in ("both", "reduced"):
+            plan = hs.hs_plan_create(N, B, Hmax, variant, out_mode)
+            got = plan.run_complex(d_F, float(scale))
+            plan.device_status()
+            ref = oracle.harmonic_sum(x, Hmax, variant)
+            what = f"complex {variant}/{out_mode}/N={N}/Hmax={Hmax}"
+            compare(plan, got, ref, what, x if out_mode == "both" else None)
+            plain = plan.run(d_x)
+            torch.cuda.synchronize()
+            if variant != "standard":                            # eq. 1's tuned kernels stage x by TMA: the direct family runs instead
+                for a, b_ in zip(got, plain):
+                    assert (a is None and b_ is None) or torch.equal(a, b_), what + ": differs from hs_execute on the same x"
+            plan.hs_destroy()
+    g = hs.hs_plan_create_ex(4096, 1, 8, "max", "full", "all", "c2")
+    with pytest.raises(hs.HsError) as e:
+        g.run_complex(torch.zeros((1, 4096, 2), device="cuda"), 1.0)
+    assert e.value.code == hs.HS_ERR_INVALID_ARG
+
+
+def test_complex_input_every_family(hs, ext, oracle):
+    N, B = 1 << 14, 4
+    F, scale = complex_batch(B, N, 77)
+    x = ext.power_spectrum(F, float(scale))
+    d_F = torch.view_as_real(torch.from_numpy(F)).contiguous().cuda()
+    for variant in VARIANTS:
+        ref = oracle.harmonic_sum(x, 32, variant)
+        for algo in ("direct", "tiled", "gather", "grouped", "twophase"):
+            plan = hs.hs_plan_create(N, B, 32, variant, "both")
+            try:
+                plan.set_algo(algo)
+            except hs.HsError:
+                continue
+            compare(plan, plan.run_complex(d_F, float(scale)), ref, f"complex {variant}/{algo}", x)
+            plan.device_status()
+
+
+def test_complex_input_sampled_at_bench_size(hs, ext, oracle):
+    """The shape bench.py --workload complex times: 1024 spectra x 2^18 bins from their Fourier series, reduced output."""
+    B, N = 1024, 1 << 18
+    g = torch.Generator(device="cuda").manual_seed(181202647 + 9)
+    d_F = torch.randn((B, N, 2), generator=g, device="cuda") * float(np.sqrt(312500.0 / 2))
+    scale = float(np.float32(1.0 / 312500.0))
+    rng = np.random.default_rng(78)
+    spectra = np.array([0, 1, 500, 1023])
+    bidx = np.concatenate([rng.choice(spectra, 1500), rng.choice(spectra, 500)])
+    nidx = np.concatenate([rng.integers(0, N, 1500), rng.integers(0, N // 32, 500)])
+    x_rows = ext.power_spectrum(d_F[spectra].cpu().numpy(), scale)
+    remap = {int(b): i for i, b in enumerate(spectra)}
+    tb, tn = torch.as_tensor(bidx, device="cuda"), torch.as_tensor(nidx, device="cuda")
+    for variant in VARIANTS:
+        plan = hs.hs_plan_create(N, B, 32, variant, "reduced")
+        _, vmax, amax = plan.run_complex(d_F, scale)
+        plan.device_status()
+        h, _ = oracle.points(x_rows, 32, variant, np.array([remap[int(b)] for b in bidx]), nidx)
+        best, second, gap, m = argmax_from_levels(h)
+        check_sums(vmax[tb, tn].cpu().numpy(), m, f"complex bench shape {variant} max")
+        check_argmax(amax[tb, tn].cpu().numpy(), best, second, gap, m, f"complex bench shape {variant} argmax")
