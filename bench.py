@@ -8,12 +8,17 @@ configuration the metric is quoted on.  `value` = bins/s, one bin = one output b
 variants x batch x nbins / step time, inputs resident in HBM; `e2e` = the same through hs_execute_host with pinned
 host buffers (host<->device copies inside the timed region).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload config2|config1|config3]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+                    [--workload config2|config1|config3|allh|plane|complex]
                     [--batch B] [--variants standard,max,freqbin,greedy] [--algo auto|direct|tiled] [--no-e2e]
 
-N > 1: launched under torchrun, one rank per GPU, every rank runs the same batch shape on its own seeded data
-(weak scaling, spectra are independent: no data-path collective); time = max over ranks.
+N > 1: one rank per GPU, every rank runs the same batch shape on its own seeded data (weak scaling, spectra are
+independent: no data-path collective); time = max over ranks.  Launched under torchrun by the driver; started plainly
+with --gpus N > 1 it re-launches itself under torch.distributed.run with N ranks (and fails if the box has fewer GPUs).
 `--impl reference` times the CPU oracle (oracle/hs_oracle.c) on a bounded sample of the same workload on rank 0.
+The non-headline workloads time the rows of SURVEY.md section 8(f): allh = every integer H up to 64 (hs_plan_create_ex),
+plane = the 2-D sum over an f-fdot plane (hs_plan_create_2d), complex = the fused power-spectrum front end
+(hs_execute_complex); each against its own algorithmic bytes.
 """
 from __future__ import annotations
 
@@ -36,8 +41,14 @@ WORKLOADS = {
     "config2": (4096, 1 << 18, "reduced", "configs[2]: 4096 x 2^18 Exp(1)-1 noise, 1% combs, reduced output"),
     "config1": (256, 1 << 18, "both", "configs[1] shape: 256 x 2^18, full and reduced output (Exp(1)-1 stand-in noise)"),
     "config3": (8, 1 << 23, "full", "configs[3]: 8 x 2^23 Exp(1)-1 noise, one comb each, full output"),
+    # SURVEY.md section 8(f) rows (not the headline): Exp(1)-1 noise
+    "allh": (256, 1 << 18, "reduced", "8(f)-3: 256 x 2^18, every integer H = 1..64, reduced output"),
+    "plane": (8, 1 << 18, "reduced", "8(f)-4: 8 f-fdot planes of 129 drifts x 2^18 bins, 2-D sum, Hmax 32, reduced output"),
+    "complex": (1024, 1 << 18, "reduced", "8(f)-1: 1024 x 2^18 complex Fourier series -> |F|^2 -> harmonic sum, Hmax 32, reduced output"),
 }
+PLANE_ROWS = 129
 BYTES_PER_BIN = {"reduced": 4 + 5, "full": 4 + 4 * 6, "both": 4 + 4 * 6 + 5}   # SURVEY.md section 8(d), Hmax = 32
+PAPER_GPU_OVER_CPU = {"standard": 250, "greedy": 704, "freqbin": 110, "max": 177}   # PAPER.md:66-71, Table 1 (hardware not stated)
 
 
 def parse():
@@ -116,6 +127,38 @@ class ClockSampler:
                     reasons.add(name)
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
                 "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_per_variant(x_rows, variants, threads, gpu_bins_per_s):
+    """the oracle's bins/s per variant on 1 thread (one spectrum) and spectra-parallel on all host
+    threads (the paper's CPU strategy), beside the paper's Table 1 ratios."""
+    import oracle
+    oracle.build()
+    R, N = x_rows.shape
+    out = {}
+    for v in variants:
+        t0 = time.perf_counter()
+        oracle.harmonic_sum(x_rows[0], 32, v, want_sums=False, want_reduced=True)
+        one = N / (time.perf_counter() - t0)
+        rows = min(R, threads)
+        t0 = time.perf_counter()
+        with concurrent.futures.ThreadPoolExecutor(max_workers=threads) as ex:
+            list(ex.map(lambda r: oracle.harmonic_sum(x_rows[r], 32, v, want_sums=False, want_reduced=True), range(rows)))
+        allc = rows * N / (time.perf_counter() - t0)
+        out[v] = {"bins_per_s_1_thread": one, "bins_per_s_all_threads": allc, "spectra_timed": rows,
+                  "gpu_over_cpu_all_threads": (gpu_bins_per_s[v] / allc) if v in gpu_bins_per_s else None,
+                  "paper_gpu_over_cpu": PAPER_GPU_OVER_CPU.get(v)}
+    return out
 
 
 def oracle_rate(x_rows, variants, seconds, threads):
@@ -250,6 +293,19 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started plainly: one rank per GPU under torch.distributed.run, or a clean failure (never an n_gpus: 1 line)
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            print(json.dumps({"error": f"--gpus {args.gpus} asked for, {have} CUDA device(s) visible", "n_gpus": have}), flush=True)
+            sys.exit(2)
+        port = 29500 + (os.getpid() % 2000)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
+    if args.gpus != world:
+        print(json.dumps({"error": f"--gpus {args.gpus} but WORLD_SIZE is {world}"}), flush=True)
+        sys.exit(2)
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
@@ -259,33 +315,56 @@ def main():
     if args.batch:
         batch = args.batch
     variants = args.variants.split(",")
-    L = 6
+    headline_workload = args.workload in ("config2", "config1", "config3")
+    wl = args.workload
+    if wl == "plane":
+        variants = [v for v in variants if v in ("standard", "freqbin")]      # the 2-D sum is defined for eqs. 1 and 3
+    Hmax = 64 if wl == "allh" else 32
+    L = 64 if wl == "allh" else 6
+    rows = PLANE_ROWS if wl == "plane" else 1                                   # rows of one batch entry
+    bins_per_entry = nbins * rows
 
     # ---- inputs, resident in HBM (seeded; every rank draws its own batch: weak scaling) -----------------------------
-    cfg = {"config2": 2, "config1": 2, "config3": 3}[args.workload]
-    x = W.exp_noise_torch(batch, nbins, cfg + 100 * rank, dev)
-    if args.workload == "config3":
-        W.inject_combs_torch(x, 3, 1.0, 1000.0, 100000.0, 0.03)
+    cfg = {"config2": 2, "config1": 2, "config3": 3, "allh": 5, "plane": 6, "complex": 7}[wl]
+    scale = float(np.float32(1.0 / 312500.0))
+    if wl == "complex":
+        g = torch.Generator(device=dev).manual_seed(W.S0 + cfg + 100 * rank)
+        x = torch.randn((batch, nbins, 2), generator=g, device=dev) * float(np.sqrt(312500.0 / 2))   # |F|^2 scale ~ Exp(1)
     else:
-        W.inject_combs_torch(x, 2, 0.01, 50.0, 5000.0, 0.10)
-    sums = torch.empty((batch, L, nbins), dtype=torch.float32, device=dev) if out_mode in ("full", "both") else None
-    vmax = torch.empty((batch, nbins), dtype=torch.float32, device=dev) if out_mode in ("reduced", "both") else None
-    amax = torch.empty((batch, nbins), dtype=torch.uint8, device=dev) if out_mode in ("reduced", "both") else None
+        x = W.exp_noise_torch(batch * rows, nbins, cfg + 100 * rank, dev)
+        if wl == "config3":
+            W.inject_combs_torch(x, 3, 1.0, 1000.0, 100000.0, 0.03)
+        elif wl in ("config2", "config1"):
+            W.inject_combs_torch(x, 2, 0.01, 50.0, 5000.0, 0.10)
+        if rows > 1:
+            x = x.view(batch, rows, nbins)
+    oshape = (batch, nbins) if rows == 1 else (batch, rows, nbins)
+    sums = torch.empty((batch, L) + oshape[1:], dtype=torch.float32, device=dev) if out_mode in ("full", "both") else None
+    vmax = torch.empty(oshape, dtype=torch.float32, device=dev) if out_mode in ("reduced", "both") else None
+    amax = torch.empty(oshape, dtype=torch.uint8, device=dev) if out_mode in ("reduced", "both") else None
     plans = {}
     for v in variants:
-        p = hs.hs_plan_create(nbins, batch, 32, v, out_mode)
-        ok = not (args.algo in ("twophase", "grouped") and v not in ("max", "freqbin")) and not (args.algo == "gather" and v not in ("freqbin", "greedy"))
-        p.set_algo(args.algo if ok else "auto")
+        if wl == "allh":
+            p = hs.hs_plan_create_ex(nbins, batch, Hmax, v, out_mode, "all", "c2")
+        elif wl == "plane":
+            p = hs.hs_plan_create_2d(nbins, rows, batch, Hmax, v, out_mode)
+        else:
+            p = hs.hs_plan_create(nbins, batch, 32, v, out_mode)
+            ok = not (args.algo in ("twophase", "grouped") and v not in ("max", "freqbin")) and not (args.algo == "gather" and v not in ("freqbin", "greedy"))
+            p.set_algo(args.algo if ok else "auto")
         p.ensure_workspace(dev)
         plans[v] = p
-    algo_names = {hs.HS_ALGO_DIRECT: "direct", hs.HS_ALGO_TILED: "tiled"}
+    algo_names = {hs.HS_ALGO_DIRECT: "direct", hs.HS_ALGO_TILED: "tiled", hs.HS_ALGO_GENERAL: "general"}
     stream = torch.cuda.current_stream()
 
     def step(events=None):
         for v in variants:
             if events is not None:
                 events[v][0].record(stream)
-            plans[v].hs_execute(x, sums, vmax, amax, stream)
+            if wl == "complex":
+                plans[v].hs_execute_complex(x, scale, sums, vmax, amax, stream)
+            else:
+                plans[v].hs_execute(x, sums, vmax, amax, stream)
             if events is not None:
                 events[v][1].record(stream)
 
@@ -310,25 +389,28 @@ def main():
         dist.barrier()
     torch.cuda.synchronize()
     clocks = sampler.stop() if sampler else None
+    for v in variants:
+        plans[v].device_status(stream)                       # no kernel of the timed region gave up a wait (else it raises)
     local_ms = ev0.elapsed_time(ev1)
     total_ms = max_over_ranks_ms(local_ms, dist if world > 1 else None)
     ms_per_step = total_ms / args.steps
-    bins_per_step = float(len(variants)) * batch * nbins * world
+    bins_per_step = float(len(variants)) * batch * bins_per_entry * world
     value = bins_per_step / (ms_per_step * 1e-3)
 
     per_variant_ms = {v: statistics.mean(e[v][0].elapsed_time(e[v][1]) for e in per_step_events) for v in variants}
     per_variant_best = {v: min(e[v][0].elapsed_time(e[v][1]) for e in per_step_events) for v in variants}
     peak, peak_src = measured_peak()
-    bpb = BYTES_PER_BIN[out_mode]
+    bpb = BYTES_PER_BIN[out_mode] if headline_workload else {"allh": 4 + 5, "plane": 4 + 5, "complex": 8 + 5}[wl]
+    nbins_eff = bins_per_entry                               # output bins per batch entry
     per_variant = {}
     default_kernels = {"standard": "rb_kernel", "max": "gr_kernel", "freqbin": "il_persistent_kernel",
                        "greedy": "hs_greedy_gather_kernel"}
     WAIT_WORDS = {"gr_kernel": "[group-barrier waits that had to spin, polls, -, -]",
                   "il_persistent_kernel": "[times a CTA found neither of its tickets runnable, polls of those, -, -]"}
     for v in variants:
-        gbs = bpb * batch * nbins / (per_variant_ms[v] * 1e-3) / 1e9
+        gbs = bpb * batch * nbins_eff / (per_variant_ms[v] * 1e-3) / 1e9
         per_variant[v] = {"ms": per_variant_ms[v], "best_ms": per_variant_best[v],
-                          "bins_per_s": batch * nbins / (per_variant_ms[v] * 1e-3), "eff_GBps": gbs,
+                          "bins_per_s": batch * nbins_eff / (per_variant_ms[v] * 1e-3), "eff_GBps": gbs,
                           "frac_of_measured_peak": gbs / peak, "frac_of_nominal_8TBps": gbs / 8000.0,
                           "algo": algo_names[plans[v].algo], "launches": plans[v].launches()}
         ws = plans[v]._ws
@@ -341,10 +423,17 @@ def main():
     dominant = max(variants, key=lambda v: per_variant_ms[v])
     dom_algo = per_variant[dominant]["algo"]
     kname = default_kernels[dominant] if (args.algo == "auto" and args.workload == "config2") else dom_algo
+    if wl in ("allh", "plane"):
+        kname = "hs_allh_kernel" if wl == "allh" else "hs_2d_kernel"
+    traffic = ncu_traffic(dominant, args.workload, dom_algo)
     roofline = {"bound": "hbm", "kernel": f"{kname} ({dominant}, eq. {1 + VARIANTS.index(dominant) if dominant in VARIANTS else 0})", "achieved": per_variant[dominant]["eff_GBps"],
                 "peak": peak, "unit": "GB/s", "frac": per_variant[dominant]["eff_GBps"] / peak,
-                "traffic": ncu_traffic(dominant, args.workload, dom_algo),
-                "algorithmic_bytes_per_launch": bpb * batch * nbins, "peak_source": peak_src}
+                "traffic": traffic,
+                "traffic_source": ("profiles/ncu_traffic.json: dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full "
+                                   "capture of this kernel on this workload (re-captured whenever a default kernel changes; "
+                                   "not measured in this run)") if traffic is not None else None,
+                "algorithmic_bytes_per_launch": bpb * batch * nbins_eff, "algorithmic_bytes_per_bin": bpb,
+                "peak_source": peak_src}
 
     if rank != 0 and world > 1:
         # other ranks still take part in the e2e collectives below
@@ -352,7 +441,7 @@ def main():
 
     # ---- fused back end: hs_execute_candidates, 4 B/bin of HBM traffic instead of 9 -------------------
     cand_line = None
-    if out_mode == "reduced" and args.candidates_threshold > 0:
+    if out_mode == "reduced" and args.candidates_threshold > 0 and headline_workload:
         cap = 1 << 22
         d_cand = torch.empty((cap, 4), dtype=torch.int32, device=dev)
         d_count = torch.zeros(1, dtype=torch.int64, device=dev)
@@ -374,7 +463,9 @@ def main():
 
     # ---- e2e: the same step through hs_execute_host with pinned host buffers -------------------------------------------
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not headline_workload:
+        e2e = {"value": None, "unit": "bins/s", "unavailable": "the end-to-end leg is timed on the headline workloads only"}
+    elif not args.no_e2e:
         ok, why = 1, ""
         try:
             slab = max(1, min(batch, (1 << 26) // nbins))          # 256 MiB of input per slab
@@ -424,26 +515,29 @@ def main():
 
     # ---- cpu_baseline: the oracle on a bounded sample of the same workload (rank 0, N = 1 only) ------------------------
     cpu = None
-    if rank == 0 and world == 1 and args.cpu_seconds > 0:
+    if rank == 0 and world == 1 and args.cpu_seconds > 0 and headline_workload:
         threads = os.cpu_count() or 1
-        rows = cpu_sample_rows(args.cpu_seconds, threads, nbins, variants)
-        rows = min(rows, batch)
-        x_rows = x[:rows].cpu().numpy()
+        crows = cpu_sample_rows(args.cpu_seconds, threads, nbins, variants)
+        crows = min(crows, batch)
+        x_rows = x[:crows].cpu().numpy()
         rate, dt, done = oracle_rate(x_rows, variants, args.cpu_seconds, threads)
         cpu = {"value": rate, "unit": "bins/s", "cores": threads, "kind": "oracle",
-               "sample": f"first {rows} spectra of the batch x {len(variants)} variants, whole spectra, {dt:.1f} s",
-               "gpu_over_cpu": value / rate}
+               "sample": f"first {crows} spectra of the batch x {len(variants)} variants, whole spectra, {dt:.1f} s",
+               "gpu_over_cpu": value / rate, "cpu_model": cpu_model(),
+               "flags": "gcc -std=c99 -O2 (no -ffast-math), fp64, one spectrum per task (PAPER.md:27)",
+               "per_variant": oracle_per_variant(x_rows, variants, threads, {v: per_variant[v]["bins_per_s"] for v in variants}),
+               "paper_context": "PAPER.md:66-71 Table 1 GPU/CPU speed-ups (hardware not stated): standard 250x, Greedy 704x, freq-bin 110x, Max 177x"}
 
     if rank == 0:
         line = {"metric": "harmonic_sum_bins_per_s", "value": value, "unit": "bins/s", "n_gpus": world,
-                "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_per_step,
+                "steps": args.steps, "warmup": max(3, args.warmup), "warmup_requested": args.warmup, "ms_per_step": ms_per_step,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": desc, "batch_per_gpu": batch, "nbins": nbins, "Hmax": 32, "out_mode": out_mode,
+                "config": {"workload": desc, "batch_per_gpu": batch, "nbins": nbins, "Hmax": Hmax, "out_mode": out_mode,
                            "variants": variants, "algo": args.algo, "headline": not args.batch,
-                           "l2": f"input {batch * nbins * 4 / 2**20:.0f} MiB per variant launch vs 126 MB L2"
-                                 + ("" if batch * nbins * 4 > (1 << 28) else " (fits: not a headline size)"),
+                           "l2": f"input {x.numel() * 4 / 2**20:.0f} MiB per variant launch vs 126 MB L2"
+                                 + ("" if x.numel() * 4 > (1 << 28) else " (fits: not a headline size)"),
                            "parallelism": f"dp{world} (batch shards, no collective)",
-                           "input_checksum_spectrum0": W.checksum(x[:1].cpu().numpy())},
+                           "input_checksum_spectrum0": W.checksum(x[:1].reshape(1, -1)[:, :nbins].cpu().numpy())},
                 "eff_GBps": value * bpb / 1e9 / world, "frac_of_measured_peak": value * bpb / 1e9 / world / peak,
                 "frac_of_nominal_8TBps": value * bpb / 1e9 / world / 8000.0,
                 "per_variant": per_variant, "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "candidates": cand_line,

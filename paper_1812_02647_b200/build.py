@@ -36,7 +36,8 @@ def _stale(target, sources):
 def _compile(src, verbose, tuning=False):
     obj = os.path.join(OBJ, os.path.basename(src)[:-3] + (".tuning.o" if tuning else ".o"))
     if _stale(obj, [src] + _deps()):
-        cmd = [NVCC] + FLAGS + (["-DHS_TUNING"] if tuning else []) + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+        extra = (["-DHS_TUNING"] + os.environ.get("HS_TUNING_NVCC_FLAGS", "").split()) if tuning else []
+        cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")

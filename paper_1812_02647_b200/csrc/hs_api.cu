@@ -94,7 +94,8 @@ slab_layout layout_of(const hs_plan *p, int64_t slab)
     s.sums = (p->out_mode & HS_OUT_FULL) ? round_up(bins * 4 * p->L, 256) : 0;
     s.vmax = (p->out_mode & HS_OUT_REDUCED) ? round_up(bins * 4, 256) : 0;
     s.amax = (p->out_mode & HS_OUT_REDUCED) ? round_up(bins, 256) : 0;
-    s.ws = p->algo == HS_ALGO_TILED ? round_up(hs_tiled_workspace_bytes(p, slab), 256) : 0;
+    s.ws = p->algo == HS_ALGO_TILED ? round_up(hs_tiled_workspace_bytes(p, slab), 256)
+         : p->algo == HS_ALGO_GENERAL ? round_up(hs_general_workspace_bytes(p), 256) : 0;
     s.total = s.x + s.sums + s.vmax + s.amax + s.ws;
     return s;
 }
@@ -243,6 +244,7 @@ int hs_plan_set_algo(hs_plan *p, int algo)
 size_t hs_plan_workspace_bytes(const hs_plan *p)
 {
     if (!p) return 0;
+    if (p->algo == HS_ALGO_GENERAL) return hs_general_workspace_bytes(p);
     return p->algo == HS_ALGO_TILED ? hs_tiled_workspace_bytes(p, p->batch) : 0;
 }
 
@@ -267,7 +269,7 @@ int hs_plan_launches(const hs_plan *p)
 {
     if (!p) return -1;
     if (p->algo == HS_ALGO_TILED) return hs_tiled_launches(p, p->batch);
-    if (p->algo == HS_ALGO_GENERAL) return (int)((p->batch + 65534) / 65535);
+    if (p->algo == HS_ALGO_GENERAL) return hs_general_workspace_bytes(p) ? 2 : (int)((p->batch + 65534) / 65535);
     const int64_t tiles = (p->nbins + 255) / 256;
     const int64_t max_spectra = ((int64_t)1 << 30) / tiles;
     return (int)((p->batch + max_spectra - 1) / max_spectra);

@@ -250,9 +250,17 @@ int d2_by_level(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStre
 
 }  // namespace
 
-int hs_launch_general(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *, cudaStream_t stream)
+// The 2-D standard sum at Hmax 32 with reduced output on rows of whole 4096-bin tiles is eq. 1's register-blocked kernel
+// with each harmonic's window taken from the plane row of its drift (hs_standard_rb.cu); it needs that kernel's tile counter.
+size_t hs_general_workspace_bytes(const hs_plan *p)
+{
+    return (p->nz > 1 && hs_standard_rb_supported(p)) ? hs_standard_rb_workspace_bytes(p) : 0;
+}
+
+int hs_launch_general(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)
 {
     if (p->nz > 1) {
+        if (hs_standard_rb_supported(p) && !buf.sink.cand) return hs_standard_rb_launch(p, buf, batch, ws, stream);
         if (p->variant == HS_STANDARD) return d2_by_level<HS_STANDARD>(p, buf, batch, stream);
         return d2_by_level<HS_FREQBIN>(p, buf, batch, stream);
     }

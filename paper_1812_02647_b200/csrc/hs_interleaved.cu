@@ -37,6 +37,9 @@
 
 namespace {
 
+#ifndef HS_IL_CTAS
+#define HS_IL_CTAS 2
+#endif
 #ifndef HS_IL_G
 #define HS_IL_G 16
 #endif
@@ -49,7 +52,10 @@ constexpr int kWarpBins = (32 / kLPR) * C;              // bins per warp
 constexpr int kGTile = kWarps * kWarpBins;              // 256 bins per gather tile
 constexpr int kGSub = 3;                                // tiles per G item above the heavy region (bins >= N/8), 1 below
                                                         // (B200: 1 -> 4.03 ms, 2 -> 3.84, 3 -> 3.76, 4 -> 3.73 with waits, 8 -> 5.2)
-constexpr int kTBins = 512 * 16 / G;                    // bins per T item (32 KiB of input)
+#ifndef HS_IL_TBINS
+#define HS_IL_TBINS 512
+#endif
+constexpr int kTBins = HS_IL_TBINS * 16 / G;            // bins per T item (32 KiB of input)
 constexpr int kTStride = kTBins + 4;                    // shared-memory row stride (floats) of the copy tile
 constexpr int kMaxRing = 3;
 
@@ -330,7 +336,7 @@ using il_tickets = hssync::tickets;
 constexpr int kItemG = 1 << 30;
 
 template <int L, int OUT, bool CPLX>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, HS_IL_CTAS)
 il_persistent_kernel(const __grid_constant__ il_params p)
 {
     __shared__ __align__(16) float tile[G * kTStride];
@@ -400,7 +406,7 @@ struct il_sched {
     int groups, R, nT, nG, nHeavy, gsub, n_split;
     int64_t slot_words;
 };
-constexpr int kCtasPerSm = 2;                                           // (__launch_bounds__ of the kernel)
+constexpr int kCtasPerSm = HS_IL_CTAS;                                  // (__launch_bounds__ of the kernel)
 
 il_sched make_sched(const hs_plan *p, int64_t batch)
 {

@@ -58,6 +58,8 @@ struct rb_params {
     int N;
     int tiles_per_spectrum;
     int tiles;       // total (< 2^31: checked on the host)
+    int Z;           // rows of an f-fdot plane (hs_plan_create_2d): a "spectrum" is then one plane row zi, and harmonic i of
+                     // drift z = zi - (Z-1)/2 reads row floor((z i + 16)/32) of the same plane; 1 = the one-dimensional sum
 };
 
 __device__ __forceinline__ void cp_async16(void *dst, const void *src)
@@ -166,7 +168,15 @@ rb_kernel(const __grid_constant__ rb_params p)
         constexpr int SC = decltype(sc)::value, IA = stream_a(SC), IB = stream_b(SC);
         if (live) {
             float *dst = ring + islot * kSlot;
-            const float *xb = p.x + ((int64_t)ib * N + (int64_t)it * (kT / 32 * IA));        // x[n0 IA / 32]: 16-byte aligned
+            // the row harmonic IA (and IB) of "spectrum" ib is read from: ib itself, or in the 2-D sum the plane row at
+            // drift floor((z i + 16) / 32) (arithmetic shift: floor toward minus infinity)
+            auto src_row = [&](int i) -> int64_t {
+                if (p.Z == 1) return ib;
+                const int Zc = (p.Z - 1) >> 1, pl = ib / p.Z, z = ib - pl * p.Z - Zc;
+                return (int64_t)pl * p.Z + ((z * i + 16) >> 5) + Zc;
+            };
+            const float *xb = p.x + (src_row(IA) * N + (int64_t)it * (kT / 32 * IA));        // x[n0 IA / 32]: 16-byte aligned
+            const float *xb2 = p.x + (src_row(IB == 0 ? IA : IB) * N + (int64_t)it * (kT / 32 * (IB == 0 ? IA : IB)));
             if constexpr (is_padded(IA)) {
                 auto copy_padded = [&](auto ic, float *d, const float *src) {
                     constexpr int I = decltype(ic)::value, units = 32 * I + (I <= 16 ? 1 : 0), rowu = I / 4;
@@ -178,14 +188,13 @@ rb_kernel(const __grid_constant__ rb_params p)
                 };
                 copy_padded(std::integral_constant<int, IA>{}, dst, xb);
                 if constexpr (IB != 0)
-                    copy_padded(std::integral_constant<int, IB == 0 ? 8 : IB>{}, dst + slot_words(IA),
-                                xb + (int64_t)it * (kT / 32 * (IB - IA)));
+                    copy_padded(std::integral_constant<int, IB == 0 ? 8 : IB>{}, dst + slot_words(IA), xb2);
             } else if (threadIdx.x == 0) {
                 constexpr uint32_t bytesA = (uint32_t)slot_words(IA) * 4u, bytesB = (uint32_t)slot_words(IB) * 4u;
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the slot was last read by ordinary loads
                 hsptx::mbar_arrive_expect_tx(&full[islot], bytesA + bytesB);
                 hsptx::bulk_g2s(dst, xb, bytesA, &full[islot]);
-                hsptx::bulk_g2s(dst + slot_words(IA), xb + (int64_t)it * (kT / 32 * (IB - IA)), bytesB, &full[islot]);
+                hsptx::bulk_g2s(dst + slot_words(IA), xb2, bytesB, &full[islot]);
             }
         }
         cp_async_commit();
@@ -270,11 +279,12 @@ rb_kernel(const __grid_constant__ rb_params p)
 
 }  // namespace
 
-// Hmax = 32, reduced output only, spectra made of whole 4096-bin tiles; everything else takes hs_standard_tiled.cu.
+// Hmax = 32, reduced output only, spectra made of whole 4096-bin tiles; everything else takes hs_standard_tiled.cu
+// (or, for the 2-D sum, hs_general.cu).
 bool hs_standard_rb_supported(const hs_plan *p)
 {
     return p->variant == HS_STANDARD && p->Hmax == 32 && p->out_mode == HS_OUT_REDUCED && p->nbins % kT == 0 &&
-           p->batch * (p->nbins / kT) < ((int64_t)1 << 30);
+           p->levels_mode == HS_LEVELS_DYADIC && p->batch * p->nz * (p->nbins / kT) < ((int64_t)1 << 30);
 }
 
 size_t hs_standard_rb_workspace_bytes(const hs_plan *) { return 512; }   // the tile counter (one 256-byte line, padded)
@@ -288,7 +298,8 @@ int hs_standard_rb_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch
     prm.amax = buf.amax;
     prm.N = (int)p->nbins;
     prm.tiles_per_spectrum = (int)(p->nbins / kT);
-    prm.tiles = (int)(batch * prm.tiles_per_spectrum);
+    prm.tiles = (int)(batch * p->nz * prm.tiles_per_spectrum);
+    prm.Z = (int)p->nz;
     prm.counter = static_cast<int *>(ws);
     prm.sink = buf.sink;
     const size_t smem = (size_t)(kSlots * kSlot) * sizeof(float);
