@@ -131,7 +131,7 @@ bool hs_tiled_supports_complex(const hs_plan *p);   // the resolved kernel start
 
 // ---- fused front end (hs_execute_complex) ----------------------------------------------------
 // x(k) = (re^2 + im^2) * scale - 1, fp32, every operation rounded on its own (the _rn intrinsics are never contracted
-// into a fused multiply-add): bit-identical to oracle/hs_oracle_ext.c hsx_power_spectrum, so that the comparisons the
+// into a fused multiply-add): bit-identical to the definition the parity tests check against (separately rounded fp32 operations), so that the comparisons the
 // harmonic sum takes on x (Greedy's drift, the best level) are the same on both sides.
 __device__ __forceinline__ float hs_power(float re, float im, float scale)
 {

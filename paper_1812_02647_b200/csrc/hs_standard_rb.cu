@@ -135,7 +135,9 @@ __device__ __forceinline__ void for_each_stage(F &f, std::integer_sequence<int, 
     (f(std::integral_constant<int, s>{}), ...);
 }
 
-template <bool CAND>
+// PLANE: the two-dimensional sum (p.Z > 1); a compile-time switch so that the one-dimensional kernel carries none of the
+// row arithmetic (it cost 11 % there when it was a run-time test).
+template <bool CAND, bool PLANE>
 __global__ void __launch_bounds__(kNT, kCtasPerSm)
 rb_kernel(const __grid_constant__ rb_params p)
 {
@@ -171,12 +173,13 @@ rb_kernel(const __grid_constant__ rb_params p)
             // the row harmonic IA (and IB) of "spectrum" ib is read from: ib itself, or in the 2-D sum the plane row at
             // drift floor((z i + 16) / 32) (arithmetic shift: floor toward minus infinity)
             auto src_row = [&](int i) -> int64_t {
-                if (p.Z == 1) return ib;
+                if constexpr (!PLANE) return ib;
                 const int Zc = (p.Z - 1) >> 1, pl = ib / p.Z, z = ib - pl * p.Z - Zc;
                 return (int64_t)pl * p.Z + ((z * i + 16) >> 5) + Zc;
             };
             const float *xb = p.x + (src_row(IA) * N + (int64_t)it * (kT / 32 * IA));        // x[n0 IA / 32]: 16-byte aligned
-            const float *xb2 = p.x + (src_row(IB == 0 ? IA : IB) * N + (int64_t)it * (kT / 32 * (IB == 0 ? IA : IB)));
+            const float *xb2 = PLANE ? p.x + (src_row(IB == 0 ? IA : IB) * N + (int64_t)it * (kT / 32 * (IB == 0 ? IA : IB)))
+                                     : xb + (int64_t)it * (kT / 32 * (IB - IA));
             if constexpr (is_padded(IA)) {
                 auto copy_padded = [&](auto ic, float *d, const float *src) {
                     constexpr int I = decltype(ic)::value, units = 32 * I + (I <= 16 ? 1 : 0), rowu = I / 4;
@@ -304,13 +307,14 @@ int hs_standard_rb_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch
     prm.sink = buf.sink;
     const size_t smem = (size_t)(kSlots * kSlot) * sizeof(float);
     // (function attributes are per device: set on every launch rather than once per process)
-    if (buf.sink.cand) HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    else HS_CUDA_OK(cudaFuncSetAttribute(rb_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const bool plane = p->nz > 1;
+    auto kern = buf.sink.cand ? (plane ? rb_kernel<true, true> : rb_kernel<true, false>)
+                              : (plane ? rb_kernel<false, true> : rb_kernel<false, false>);
+    HS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t slots = (int64_t)p->sm_count * kCtasPerSm;
     const unsigned grid = (unsigned)(prm.tiles < slots ? prm.tiles : slots);
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, 256, stream));
-    if (buf.sink.cand) rb_kernel<true><<<grid, kNT, smem, stream>>>(prm);
-    else rb_kernel<false><<<grid, kNT, smem, stream>>>(prm);
+    kern<<<grid, kNT, smem, stream>>>(prm);
     HS_CUDA_OK(cudaGetLastError());
     return HS_OK;
 }
