@@ -19,18 +19,20 @@
 //     T item: copy 512 bins x 16 spectra of a group into its ring slot; bins n >= N/2 have no harmonic but the first in
 //             range (S_H(n) = x(n) for every H), so their outputs are emitted right here, in the natural layout;
 //     G item: the gather for 256 bins (x 1 below N/8, x 3 above) x 16 spectra of a group, low (= long) bins first.
-// Thread 0 of a CTA holds up to one ticket of each queue (fetch-and-add) and runs whichever is runnable, gathers first:
-// a G ticket once ALL T items of its group are complete, a T ticket once the gather of the group that used its ring slot
-// last (g - R) is complete.  A ticket that is not runnable is kept while the other kind of work goes on, so no CTA
-// ever waits inside an item, a slow gather phase throttles the copies without parking CTAs on them (the static
-// "[T(s)][G(s-1)]" order of round 1 parked CTAs on copy items whenever the gathers fell behind), and the ring only has
-// to hold the groups in flight (R slots).  Replacement tickets are drawn while the current item's first loads are in flight.
+// A CTA is eight worker warps and one SCHEDULER warp (one active lane).  The scheduler holds up to one ticket of each
+// queue (fetch-and-add) and picks whichever is runnable, gathers first: a G ticket once ALL T items of its group are
+// complete, a T ticket once the gather of the group that used its ring slot last (g - R) is complete; a ticket that is
+// not runnable is kept while the other kind of work goes on.  It does this WHILE the workers run the previous item:
+// it publishes item k + 1 in a shared-memory mailbox, draws the replacement ticket, starts the TMA bulk copies of a T
+// ticket's input rows into one of two shared-memory tiles (x is read only, so this needs nothing but the ticket
+// number), and when the workers report item k done it releases its completion at gpu scope (fence + the group's
+// counter).  Measured with thread 0 doing all of this between items: release 0.7 - 0.8 us + choice 1.0 us per item on
+// top of item bodies of 2.6 us (T) and 6.5 us (G); with the scheduler warp 3.92 -> 3.63 ms (profiles/r02_il_items.md).
 //
 // Gather thread = (4 spectra of the group, C = 4 consecutive bins): one 16-byte load per bin and harmonic serves four
 // spectra, the outputs of a thread are four float4 and four 4-byte stores; a warp owns 32 consecutive bins.  Range
-// handling is warp-uniform: harmonic i is in range for every lane iff i (n_hi + 1) <= N.  Ring data is read with
-// ordinary (L1-allocating) loads: every CTA's first read of a group follows its own acquire of the group's counter,
-// which invalidates the SM's L1 (SASS: CCTL.IVALL).
+// handling is warp-uniform: harmonic i is in range for every lane iff i (n_hi + 1) <= N.  The loads of harmonic i + 2
+// are issued (cp.async into a per-thread shared-memory FIFO) before harmonic i is consumed: no staging registers.
 #include "hs_internal.cuh"
 #include "hs_ptx.cuh"
 #include "hs_sync.cuh"
@@ -58,6 +60,11 @@ constexpr int kGSub = 3;                                // tiles per G item abov
 constexpr int kTBins = HS_IL_TBINS * 16 / G;            // bins per T item (32 KiB of input)
 constexpr int kTStride = kTBins + 4;                    // shared-memory row stride (floats) of the copy tile
 constexpr int kMaxRing = 3;
+#ifndef HS_IL_DEPTH
+#define HS_IL_DEPTH 2
+#endif
+constexpr int kDepth = HS_IL_DEPTH;                     // harmonics in flight per gather thread (cp.async into a per-thread FIFO)
+constexpr size_t kFifoBytes = (size_t)kDepth * C * kThreads * sizeof(float4);
 
 struct il_params {
     const float *x;
@@ -88,8 +95,44 @@ __device__ __forceinline__ float4 ld_stream(const float4 *p)   // read-once inpu
     asm volatile("ld.global.cs.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
     return v;
 }
+// 16 bytes global -> shared, asynchronously; `bytes` = 16, or 0 to store zeros instead (the source is then not read)
+__device__ __forceinline__ void cp_async16(void *dst, const void *src, int bytes)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(hsptx::smem_u32(dst)), "l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void *dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(hsptx::smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait()
+{
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
 // ------------------------------------------------------------------------------------------------ T item
+// Shared-memory tile of a copy item: row g (spectrum b0 + g) holds its kTBins bins at tile + row_off(g).  The upper
+// eight rows start 8 floats later, which makes the transposed reads below conflict-free (rows are 516 floats apart).
+__device__ __forceinline__ int row_off(int g) { return g * kTStride + (g & 8); }
+constexpr int kTileFloats = G * kTStride + 8;
+
+// Start the TMA bulk copies of the input of T item (group grp, bins from k0) into `tile`: one copy per spectrum row that
+// exists, the part of it below N; completion on `bar`.  One thread.  x is read only: this may run long before the item.
+__device__ __forceinline__ void prefetch_item(const il_params &p, float *tile, uint64_t *bar, int grp, int k0)
+{
+    const int64_t b0 = (int64_t)grp * G;
+    const int nb = (int)min((int64_t)G, (int64_t)p.B - b0);
+    const int cols = min(kTBins, p.N - k0);                              // multiple of 4 (N % 4 == 0)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");         // the tile was last read by ordinary loads
+    hsptx::mbar_arrive_expect_tx(bar, (uint32_t)nb * (uint32_t)cols * 4u);
+    const uint64_t pol = hsptx::policy_evict_first();                    // read once: must not push the ring out of L2
+    for (int g = 0; g < nb; g++)
+        hsptx::bulk_g2s_hint(tile + row_off(g), p.x + (b0 + g) * p.N + k0, (uint32_t)cols * 4u, bar, pol);
+}
+
 // xT[k][g] = x[b0 + g][k] for g < nb, 0 for nb <= g < G, k in [k0, k0 + 512) below N; outputs of the bins >= n_split.
+// The input is in `tile` already (prefetch_item, waited for by the caller) unless CPLX: the fused front end forms
+// x = |F|^2 scale - 1 here while loading, and x is never written to HBM.
 template <int L, int OUT, bool CPLX, class F>
 __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int grp, int k0, float *__restrict__ xT, F &redraw)
 {
@@ -105,16 +148,16 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
         const int g = warp * SPW + s;
 #pragma unroll
         for (int q = 0; q < Q; q++) {
-            const int k = k0 + 4 * (lane + 32 * q);
+            const int kk = 4 * (lane + 32 * q), k = k0 + kk;
             v[s][q] = make_float4(0.f, 0.f, 0.f, 0.f);
             if (g < nb && k < N) {
-                if (CPLX) {                               // the fused front end: x is formed here and never written to HBM
+                if (CPLX) {
                     const float4 *f = reinterpret_cast<const float4 *>(p.x + ((b0 + g) * N + k) * 2);
                     const float4 a = ld_stream(f), c = ld_stream(f + 1);
                     v[s][q] = make_float4(hs_power(a.x, a.y, p.scale), hs_power(a.z, a.w, p.scale),
                                           hs_power(c.x, c.y, p.scale), hs_power(c.z, c.w, p.scale));
                 } else {
-                    v[s][q] = ld_stream(reinterpret_cast<const float4 *>(p.x + (b0 + g) * N + k));
+                    v[s][q] = *reinterpret_cast<const float4 *>(tile + row_off(g) + kk);
                 }
             }
         }
@@ -126,8 +169,7 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
 #pragma unroll
         for (int q = 0; q < Q; q++) {
             const int kk = 4 * (lane + 32 * q);
-            // bit 3 of the column is flipped for the upper 8 spectra: makes the transposed reads below conflict-free
-            *reinterpret_cast<float4 *>(tile + g * kTStride + (kk ^ (g & 8))) = v[s][q];
+            if (CPLX) *reinterpret_cast<float4 *>(tile + row_off(g) + kk) = v[s][q];
             const int k = k0 + kk;
             if (k >= p.n_split && k < N && g < nb) {     // S_H(n) = x(n) for every H: emit in the natural layout
                 const int64_t row = (b0 + g) * N;
@@ -161,16 +203,18 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
             }
         }
     }
-    __syncthreads();
-    // thread t writes the float4 of spectra 4 (t % 4) .. +3 at bins k0 + t / 4 + 64 q
+    if (CPLX) asm volatile("bar.sync 1, %0;" ::"n"(kThreads) : "memory");   // (the worker warps; the scheduler warp is not part of it)
+    // thread t writes the float4 of spectra 4 (t % 4) .. +3 at bins k0 + t / 4 + 64 q; rows the group does not have are zero
     const int g4 = (threadIdx.x & (kLPR - 1)) * 4;
-    const int sw = g4 & 8;
+    const float *t0 = tile + row_off(g4);
+    const int have = nb - g4;                            // rows g4 .. g4 + have - 1 exist
 #pragma unroll
     for (int q = 0; q < kTBins / (kThreads / kLPR); q++) {
         const int kk = q * (kThreads / kLPR) + (threadIdx.x / kLPR);
         if (k0 + kk < N) {
-            const float *t = tile + g4 * kTStride + (kk ^ sw);
-            const float4 o = make_float4(t[0], t[kTStride], t[2 * kTStride], t[3 * kTStride]);
+            const float *t = t0 + kk;
+            const float4 o = make_float4(have > 0 ? t[0] : 0.f, have > 1 ? t[kTStride] : 0.f, have > 2 ? t[2 * kTStride] : 0.f,
+                                         have > 3 ? t[3 * kTStride] : 0.f);
             *reinterpret_cast<float4 *>(xT + (int64_t)(k0 + kk) * G + g4) = o;
         }
     }
@@ -181,7 +225,7 @@ __device__ __forceinline__ void copy_item(const il_params &p, float *tile, int g
 // serves four spectra; a warp owns 32 consecutive bins, and per output row it stores 128 contiguous bytes of maxima
 // and 32 of best levels.
 template <int L, int OUT, class F>
-__device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_cta, const float *xT, F &redraw)
+__device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_cta, const float *xT, float4 *fifo, F &redraw)
 {
     const int N = p.N;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -242,56 +286,59 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
     };
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
 
+    // The harmonics 2 .. imax (the last one in range for some lane of the warp) are fetched kDepth ahead of their use by
+    // cp.async into a FIFO of this thread's own (stage d, bin k) -> fifo[(d C + k) kThreads + thread]: the loads in flight
+    // cost no registers, and a thread only ever reads what it copied itself (no barrier; cp.async.wait_group orders it).
+    constexpr int HM = 1 << (L - 1);
+    int imax = 1;
+    if (n_w > 0) {
+        const int q = (N - 1) / n_w;                                   // harmonic i has a bin below N for the warp iff i n_w < N
+        imax = q < HM ? q : HM;
+    } else {
+        imax = HM;
+    }
+    float4 *mine = fifo + threadIdx.x;
+    auto fetch = [&](int i) {                                          // harmonic i -> stage i % kDepth (one commit group)
+        if (i <= imax) {
+            float4 *dst = mine + (i % kDepth) * (C * kThreads);
+            const int base = i * n0;
+            if (whole && i * n_hi1 <= N) {                             // in range for every lane: no bounds checks
+#pragma unroll
+                for (int k = 0; k < C; k++) cp_async16(dst + k * kThreads, xq + (base + k * i) * RS);
+            } else {                                                   // straddling the end of the spectrum: zero padding (C5)
+#pragma unroll
+                for (int k = 0; k < C; k++) {
+                    const int r = base + k * i;
+                    cp_async16(dst + k * kThreads, xq + (r < N ? r : 0) * RS, r < N ? 16 : 0);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+#pragma unroll
+    for (int d = 0; d < kDepth; d++) fetch(2 + d);
+
     // harmonic 1
 #pragma unroll
     for (int k = 0; k < C; k++) S[k] = (whole || n0 + k < N) ? ld_ring(xq + (n0 + k) * RS) : zero;
     redraw();                                                        // (thread 0: the next item, while the loads are in flight)
     emit(0);
 
-    // harmonics i and i + 1, both in range for every lane: no bounds checks, 8 independent 16-byte loads in flight
-    auto step_safe2 = [&](int i) {
-        const int base = i * n0, base2 = base + n0;
-        float4 a[C], b[C];
-#pragma unroll
-        for (int k = 0; k < C; k++) {
-            a[k] = ld_ring(xq + (base + k * i) * RS);
-            b[k] = ld_ring(xq + (base2 + k * (i + 1)) * RS);
-        }
-#pragma unroll
-        for (int k = 0; k < C; k++) {
-            add(S[k], a[k]);
-            add(S[k], b[k]);
-        }
-    };
-    auto step_safe = [&](int i) {
-        const int base = i * n0;
-        float4 a[C];
-#pragma unroll
-        for (int k = 0; k < C; k++) a[k] = ld_ring(xq + (base + k * i) * RS);
-#pragma unroll
-        for (int k = 0; k < C; k++) add(S[k], a[k]);
-    };
-    // harmonic i straddling the end of the spectrum: zero padding (C5)
-    auto step_edge = [&](int i) {
-        const int base = i * n0;
-#pragma unroll
-        for (int k = 0; k < C; k++) {
-            const int r = base + k * i;
-            add(S[k], r < N ? ld_ring(xq + r * RS) : zero);
-        }
-    };
-
     bool tail = false;   // levels skipped because none of their harmonics is in range for the warp (reduced only)
 #pragma unroll
     for (int l = 1; l < L; l++) {
         const int lo = (1 << (l - 1)) + 1, hi = 1 << l;
-        if (lo * n_w < N) {
-            int i = lo;
-            if (whole) {
-                for (; i + 1 <= hi && (i + 1) * n_hi1 <= N; i += 2) step_safe2(i);
-                for (; i <= hi && i * n_hi1 <= N; i++) step_safe(i);
+        if (lo <= imax) {
+            for (int i = lo; i <= hi && i <= imax; i++) {
+                cp_async_wait<kDepth - 1>();                           // harmonic i has landed
+                const float4 *src = mine + (i % kDepth) * (C * kThreads);
+                float4 v[C];
+#pragma unroll
+                for (int k = 0; k < C; k++) v[k] = src[k * kThreads];
+#pragma unroll
+                for (int k = 0; k < C; k++) add(S[k], v[k]);
+                fetch(i + kDepth);                                     // refill the stage
             }
-            for (; i <= hi && i * n_w < N; i++) step_edge(i);
             emit(l);
         } else if ((OUT & 3) != HS_OUT_REDUCED) {
             emit(l);
@@ -299,6 +346,7 @@ __device__ __forceinline__ void gather_item(const il_params &p, int grp, int n_c
             tail = true;
         }
     }
+    cp_async_wait<0>();
     // With S unchanged over the skipped levels h_l = S c_l is monotone in l: testing the last level alone is enough.
     if ((OUT & 3) == HS_OUT_REDUCED && tail) emit(L - 1);
 
@@ -335,70 +383,143 @@ using hssync::kNoTicket;
 using il_tickets = hssync::tickets;
 constexpr int kItemG = 1 << 30;
 
+// CTA = 8 worker warps + 1 scheduler warp (one active lane).  The scheduler owns the tickets: while the workers run item
+// k it draws replacement tickets, starts the TMA prefetch of a T ticket's input, and picks item k + 1 (whichever ticket in
+// hand is runnable, gathers first) and publishes it; when the workers report item k done it releases the item's
+// completion at gpu scope (fence + counter) -- after the workers have already gone on to item k + 1.  None of the
+// latencies of scheduling (ticket atomics, polls of the groups' counters, the release fence: ~2 us per item, a third
+// of an item's time when thread 0 of the CTA did this between items) is on the workers' path any more.
+// If no ticket is runnable while item k is still running, the scheduler first waits for item k and releases it (item
+// k + 1 may depend on it) and only then waits for a ticket to become runnable.
 template <int L, int OUT, bool CPLX>
-__global__ void __launch_bounds__(kThreads, HS_IL_CTAS)
+__global__ void __launch_bounds__(kThreads + 32, HS_IL_CTAS)
 il_persistent_kernel(const __grid_constant__ il_params p)
 {
-    __shared__ __align__(16) float tile[G * kTStride];
-    __shared__ int s_item;
-    il_tickets q;
-    q.tq = p.ctrl + HS_CTRL_QUEUE;
-    q.gq = p.ctrl + 8;
-    q.doneT = p.ctrl + 16;
-    q.doneG = p.ctrl + 16 + p.groups;
-    q.nT = p.nT;
-    q.nG = p.nG;
-    q.R = p.R;
-    q.totalT = p.groups * p.nT;
-    q.totalG = p.groups * p.nG;
-    q.readyT = -1;
-    q.freeG = -1;                                                       // (groups below R have a fresh slot: ts - R <= -1)
-    q.gt = q.tt = kNoTicket;
-    if (threadIdx.x == 0) s_item = q.next(p.ctrl, p.spin_limit, kItemG);
+    // dynamic shared memory: the gather items' FIFO, then two tiles for the copy items (the input of the T ticket in
+    // hand is prefetched into the tile that is not in use while the CTA is busy with another item)
+    extern __shared__ __align__(128) unsigned char dyn_smem[];
+    float4 *fifo = reinterpret_cast<float4 *>(dyn_smem);
+    float *tiles = reinterpret_cast<float *>(dyn_smem + kFifoBytes);
+    __shared__ __align__(8) uint64_t tbar[2];      // a tile's input has landed (TMA)
+    // Mailboxes between the scheduler and the workers: monotonic counters (no phase parity that could be lapped)
+    __shared__ int s_done;                         // worker warps that have finished an item, summed over the items so far
+    __shared__ int s_pub;                          // items the scheduler has published
+    __shared__ int s_item[2], s_buf[2];            // item k is in slot k & 1
+    if (threadIdx.x == 0) {
+        hsptx::mbar_init(&tbar[0], 1);
+        hsptx::mbar_init(&tbar[1], 1);
+        hsptx::mbar_fence_init();
+        s_done = 0;
+        s_pub = 0;
+    }
     __syncthreads();
-    int item = s_item;
-    while (item != kNoTicket) {
-        // the ticket that replaces the one being run is drawn once this item's first loads are issued
-        auto redraw = [&]() {
-            if (threadIdx.x == 0) {
-                q.draw_g();
-                q.draw_t();
-            }
+
+    if (threadIdx.x >= kThreads) {                                      // ---------------- scheduler warp
+        if (threadIdx.x != kThreads) return;
+        il_tickets q;
+        q.tq = p.ctrl + HS_CTRL_QUEUE;
+        q.gq = p.ctrl + 8;
+        q.doneT = p.ctrl + 16;
+        q.doneG = p.ctrl + 16 + p.groups;
+        q.nT = p.nT;
+        q.nG = p.nG;
+        q.R = p.R;
+        q.totalT = p.groups * p.nT;
+        q.totalG = p.groups * p.nG;
+        q.readyT = -1;
+        q.freeG = -1;                                                   // (groups below R have a fresh slot: ts - R <= -1)
+        q.gt = q.tt = kNoTicket;
+        int pft[2] = {kNoTicket, kNoTicket};                            // the T ticket whose input is in tile b (or on its way)
+        // start the TMA copies for T ticket `t` unless it has a tile already; returns its tile, or -1 if none is free
+        auto fetch = [&](int t) -> int {
+            if (pft[0] == t) return 0;
+            if (pft[1] == t) return 1;
+            const int bsel = pft[0] == kNoTicket ? 0 : pft[1] == kNoTicket ? 1 : -1;
+            if (bsel < 0) return -1;
+            const int s = t / p.nT, idx = t - s * p.nT;
+            if (!CPLX) prefetch_item(p, tiles + bsel * kTileFloats, &tbar[bsel], s, idx * kTBins);
+            pft[bsel] = t;
+            return bsel;
         };
+        auto publish = [&](int k, int it) {                             // item number k (its parity selects the mailbox)
+            int bsel = 0;
+            if (it >= 0 && !(it & kItemG)) bsel = fetch(it);            // (a tile is free: at most one other T item is in flight)
+            *(volatile int *)&s_item[k & 1] = it;
+            *(volatile int *)&s_buf[k & 1] = bsel;
+            __threadfence_block();
+            *(volatile int *)&s_pub = k + 1;
+            q.draw_g();                                                 // replacement tickets, and the held T ticket's input
+            q.draw_t();
+            if (q.tt >= 0) (void)fetch(q.tt);
+        };
+        int cur = q.next(p.ctrl, p.spin_limit, kItemG);                 // kNoTicket: nothing to do at all
+        publish(0, cur);
+        for (int k = 0; cur != kNoTicket; k++) {
+            int nxt = q.try_next(kItemG);
+            bool published = false;
+            if (nxt != kNoTicket) {
+                if (nxt == hssync::kExhausted) nxt = kNoTicket;
+                publish(k + 1, nxt);
+                published = true;
+            }
+            while (*(volatile int *)&s_done < kWarps * (k + 1)) {       // the workers have finished item k
+            }
+            __threadfence();                                            // their stores, cumulatively, before the release at gpu scope
+            if (!(cur & kItemG)) {
+                atomicAdd(q.doneT + cur / p.nT, 1);
+                pft[pft[0] == cur ? 0 : 1] = kNoTicket;                 // (the tile has been read by everybody)
+            } else {
+                atomicAdd(q.doneG + (cur & (kItemG - 1)) / p.nG, 1);
+            }
+            if (!published) {
+                nxt = q.next(p.ctrl, p.spin_limit, kItemG);
+                publish(k + 1, nxt);
+            } else if (q.tt >= 0) {
+                (void)fetch(q.tt);                                      // (a tile may have become free)
+            }
+            cur = nxt;
+        }
+        return;
+    }
+
+    // ---------------- worker warps
+    auto nothing = []() {};
+    uint32_t tphase = 0u;                                               // bit b: parity of the next wait on tbar[b]
+    for (int k = 0;; k++) {
+        while (*(volatile int *)&s_pub <= k) {
+        }
+        __threadfence_block();
+        const int item = *(volatile int *)&s_item[k & 1], tb = *(volatile int *)&s_buf[k & 1];
+        if (item == kNoTicket) break;
         if (!(item & kItemG)) {                                         // ---- T item
             const int s = item / p.nT, idx = item - s * p.nT;
             float *xT = p.xT + (int64_t)(s % p.R) * p.slot_words;
-            copy_item<L, OUT, CPLX>(p, tile, s, idx * kTBins, xT, redraw);
-            __syncthreads();                                            // all stores of the CTA are ordered before ...
-            if (threadIdx.x == 0) {
-                __threadfence();                                        // ... thread 0's release at gpu scope
-                atomicAdd(q.doneT + s, 1);
+            if (!CPLX) {
+                hsptx::mbar_wait(&tbar[tb], (tphase >> tb) & 1u);
+                tphase ^= 1u << tb;
             }
+            copy_item<L, OUT, CPLX>(p, tiles + tb * kTileFloats, s, idx * kTBins, xT, nothing);
         } else {                                                        // ---- G item
             const int gi = item & (kItemG - 1);
             const int grp = gi / p.nG, qi = gi - grp * p.nG;
             const float *xT = p.xT + (int64_t)(grp % p.R) * p.slot_words;
             if (qi < p.nHeavy) {
-                gather_item<L, OUT>(p, grp, qi * kGTile, xT, redraw);
+                gather_item<L, OUT>(p, grp, qi * kGTile, xT, fifo, nothing);
             } else {
-                auto nothing = []() {};
 #pragma unroll 1
                 for (int sub = 0; sub < p.gsub; sub++) {
                     const int t = p.nHeavy + (qi - p.nHeavy) * p.gsub + sub;
-                    if (sub == 0) gather_item<L, OUT>(p, grp, t * kGTile, xT, redraw);
-                    else gather_item<L, OUT>(p, grp, t * kGTile, xT, nothing);
+                    gather_item<L, OUT>(p, grp, t * kGTile, xT, fifo, nothing);
                 }
             }
-            __syncthreads();                                            // every load of the slot has returned
-            if (threadIdx.x == 0) {
-                __threadfence();
-                atomicAdd(q.doneG + grp, 1);
-            }
         }
-        if (threadIdx.x == 0) s_item = q.next(p.ctrl, p.spin_limit, kItemG);
-        __syncthreads();                                                // s_item and the tile are reused
-        item = s_item;
-        __syncthreads();
+        // every load of this warp from the ring / the tile has returned (their values were consumed) and its stores are
+        // issued: one arrival per warp (release at CTA scope; the scheduler's fence makes them visible at gpu scope)
+        __syncwarp();
+        if ((threadIdx.x & 31) == 0) {
+            __threadfence_block();
+            atomicAdd(&s_done, 1);
+        }
     }
 }
 
@@ -469,13 +590,15 @@ int launch_c(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, c
     prm.gsub = s.gsub;
     prm.n_split = s.n_split;
     auto kern = il_persistent_kernel<L, OUT, CPLX>;
+    const size_t smem = kFifoBytes + 2 * (size_t)kTileFloats * sizeof(float);
+    HS_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 0;                                                        // (per device: asked on every launch)
-    HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads, 0));
+    HS_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kThreads + 32, smem));
     const int ctas_per_sm = occ > 0 ? occ : 1;
     HS_CUDA_OK(cudaMemsetAsync(ws, 0, ctrl_bytes(s.groups), stream));
     const int64_t total = (int64_t)s.groups * (s.nT + s.nG);
     const int64_t slots = (int64_t)p->sm_count * ctas_per_sm;
-    kern<<<(unsigned)(total < slots ? total : slots), kThreads, 0, stream>>>(prm);
+    kern<<<(unsigned)(total < slots ? total : slots), kThreads + 32, smem, stream>>>(prm);
     HS_CUDA_OK(cudaGetLastError());
     return HS_OK;
 }

@@ -93,6 +93,24 @@ struct tickets {
         freeG = fs;
         return true;
     }
+    // Without waiting: the next item to run (kind | index); kNoTicket if neither ticket in hand is runnable right now;
+    // kExhausted when both queues are exhausted.
+    __device__ __forceinline__ int try_next(int kItemG)
+    {
+        draw_g();
+        draw_t();
+        if (g_runnable()) {
+            const int it = kItemG | gt;
+            gt = kNoTicket;
+            return it;
+        }
+        if (t_runnable()) {
+            const int it = tt;
+            tt = kNoTicket;
+            return it;
+        }
+        return (gt == kExhausted && tt == kExhausted) ? kExhausted : kNoTicket;
+    }
     // the next item to run: kind | index, or kNoTicket when both queues are exhausted (or the poll limit was hit)
     __device__ __forceinline__ int next(int *ctrl, unsigned limit, int kItemG)
     {
