@@ -402,14 +402,15 @@ il_persistent_kernel(const __grid_constant__ il_params p)
     float *tiles = reinterpret_cast<float *>(dyn_smem + kFifoBytes);
     __shared__ __align__(8) uint64_t tbar[2];      // a tile's input has landed (TMA)
     // Mailboxes between the scheduler and the workers: monotonic counters (no phase parity that could be lapped)
-    __shared__ int s_done;                         // worker warps that have finished an item, summed over the items so far
+    __shared__ int s_done[4];                      // worker warps that have finished item k: slot k & 3 (the workers are never more
+                                                   // than one item apart, but NOT in lockstep: one counter per item, not a running sum)
     __shared__ int s_pub;                          // items the scheduler has published
     __shared__ int s_item[2], s_buf[2];            // item k is in slot k & 1
     if (threadIdx.x == 0) {
         hsptx::mbar_init(&tbar[0], 1);
         hsptx::mbar_init(&tbar[1], 1);
         hsptx::mbar_fence_init();
-        s_done = 0;
+        s_done[0] = s_done[1] = s_done[2] = s_done[3] = 0;
         s_pub = 0;
     }
     __syncthreads();
@@ -462,8 +463,9 @@ il_persistent_kernel(const __grid_constant__ il_params p)
                 publish(k + 1, nxt);
                 published = true;
             }
-            while (*(volatile int *)&s_done < kWarps * (k + 1)) {       // the workers have finished item k
+            while (*(volatile int *)&s_done[k & 3] < kWarps) {          // every worker warp has finished item k
             }
+            *(volatile int *)&s_done[k & 3] = 0;                        // (item k + 4 is published three iterations from now)
             __threadfence();                                            // their stores, cumulatively, before the release at gpu scope
             if (!(cur & kItemG)) {
                 atomicAdd(q.doneT + cur / p.nT, 1);
@@ -518,7 +520,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
         __syncwarp();
         if ((threadIdx.x & 31) == 0) {
             __threadfence_block();
-            atomicAdd(&s_done, 1);
+            atomicAdd(&s_done[k & 3], 1);
         }
     }
 }

@@ -9,6 +9,7 @@
 
 #include <cstdio>
 #include <cstdlib>
+#include <utility>
 #include <vector>
 
 namespace cg = cooperative_groups;
@@ -204,6 +205,156 @@ __global__ void ring_and_stream(float4 *ring, size_t ring_v4, const float4 *src,
     if (acc.x == 123.456f) dst[0] = acc;
 }
 
+// ---- the two dies.  die_probe: one thread per SM times a chain of dependent L2 loads (.cg) on a few fixed 128-byte lines:
+// an SM sees a line either in its own die's L2 partition or across the die link, so for every line the SMs fall into
+// two latency classes -- that is the SM -> die map.  ring_by_die: the dirty-ring test above with the ring either shared by
+// all CTAs or split into two halves that are each touched by the CTAs of ONE die only (does a die-private workspace stay
+// resident better?).
+__global__ void die_probe(unsigned *buf, int nlines, int stride_words, int iters, unsigned *out)
+{
+    extern __shared__ float die_pad[];
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    if (threadIdx.x != 0) return;
+    for (int l = 0; l < nlines; l++) {
+        unsigned *ptr = buf + (size_t)l * stride_words;
+        unsigned v;
+        asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(v) : "l"(ptr) : "memory");
+        unsigned best = 0xffffffffu;
+        for (int rep = 0; rep < 8; rep++) {
+            unsigned idx = 0;
+            const long long t0 = clock64();
+            for (int i = 0; i < iters; i++) {
+                asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(v) : "l"(ptr + idx) : "memory");
+                idx = v;                                   // the buffer holds zeros: a dependent chain on one line
+            }
+            const unsigned dt = (unsigned)(clock64() - t0);
+            if (dt < best) best = dt;
+            if (idx == 12345u) out[0] = 1;
+        }
+        out[(size_t)smid * nlines + l] = best;
+    }
+}
+
+__global__ void __launch_bounds__(512, 2)
+ring_by_die(float4 *ring, size_t ring_v4, const float4 *src, float4 *dst, size_t stream_v4, int rounds, int split,
+            const int *die, int *ticket, int ncta0, int ncta1)
+{
+    extern __shared__ float die_pad[];
+    __shared__ int s_t, s_d;
+    if (threadIdx.x == 0) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        s_d = die[smid];
+        s_t = atomicAdd(ticket + s_d, 1);
+    }
+    __syncthreads();
+    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
+    size_t rt = tid, rn = nth, r0 = 0, rlen = ring_v4;
+    if (split) {
+        rt = (size_t)s_t * blockDim.x + threadIdx.x;
+        rn = (size_t)(s_d ? ncta1 : ncta0) * blockDim.x;
+        rlen = ring_v4 / 2;
+        r0 = s_d ? rlen : 0;
+    }
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int r = 0; r < rounds; r++) {
+        for (size_t i = rt; i < rlen; i += rn) {
+            float4 v = ring[r0 + i];
+            v.x += 1.f;
+            ring[r0 + i] = v;
+        }
+        const float4 *sp = src + (size_t)r * stream_v4;
+        float4 *dp = dst + (size_t)r * stream_v4;
+        for (size_t i = tid; i < stream_v4; i += nth) {
+            float4 v;
+            asm volatile("ld.global.cs.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(sp + i));
+            acc.x += v.x;
+            asm volatile("st.global.cs.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(dp + i), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+        }
+    }
+    if (acc.x == 123.456f) dst[0] = acc;
+}
+
+void run_die_tests(int sms)
+{
+    const int nlines = 8, stride_words = 4096 * 4 + 512, iters = 64;
+    unsigned *buf, *out;
+    CK(cudaMalloc(&buf, (size_t)nlines * stride_words * 4 + 4096));
+    CK(cudaMemset(buf, 0, (size_t)nlines * stride_words * 4 + 4096));
+    CK(cudaMalloc(&out, (size_t)sms * nlines * 4));
+    CK(cudaFuncSetAttribute(die_probe, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));   // one CTA per SM
+    for (int pass = 0; pass < 2; pass++) {
+        die_probe<<<sms, 32, 200 * 1024>>>(buf, nlines, stride_words, iters, out);
+        CK(cudaDeviceSynchronize());
+    }
+    std::vector<unsigned> h((size_t)sms * nlines);
+    CK(cudaMemcpy(h.data(), out, h.size() * 4, cudaMemcpyDeviceToHost));
+    std::vector<int> die(sms, 0);
+    int n1 = 0;
+    for (int l = 0; l < 2; l++) {                          // classes by the largest gap of the sorted latencies of a line
+        std::vector<unsigned> v(sms);
+        for (int s = 0; s < sms; s++) v[s] = h[(size_t)s * nlines + l];
+        std::vector<unsigned> srt = v;
+        for (int i = 1; i < sms; i++)
+            for (int j = i; j > 0 && srt[j] < srt[j - 1]; j--) std::swap(srt[j], srt[j - 1]);
+        int cut = sms / 4;
+        unsigned gap = 0;
+        for (int i = sms / 4; i < 3 * sms / 4; i++)
+            if (srt[i] - srt[i - 1] > gap) gap = srt[i] - srt[i - 1], cut = i;
+        const unsigned thr = (srt[cut] + srt[cut - 1]) / 2;
+        int far = 0;
+        for (int s = 0; s < sms; s++) far += v[s] > thr;
+        printf("die probe, line %d: near class %5.1f .. %5.1f clk per load, far class %5.1f .. %5.1f; %d SMs near, %d far\n", l,
+               srt[0] / (float)iters, srt[cut - 1] / (float)iters, srt[cut] / (float)iters, srt[sms - 1] / (float)iters, sms - far, far);
+        if (l == 0) {
+            for (int s = 0; s < sms; s++) die[s] = v[s] > thr, n1 += die[s];
+        }
+    }
+    printf("SM -> die map from line 0 (smid order, 0 = near): ");
+    for (int s = 0; s < sms; s++) printf("%d", die[s]);
+    printf("\n");
+    int *d_die, *d_ticket;
+    CK(cudaMalloc(&d_die, sms * 4));
+    CK(cudaMalloc(&d_ticket, 8));
+    CK(cudaMemcpy(d_die, die.data(), sms * 4, cudaMemcpyHostToDevice));
+    const int cps = 2, smem = 100 * 1024, rounds = 16;     // exactly two CTAs per SM
+    CK(cudaFuncSetAttribute(ring_by_die, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    for (size_t ring_mib : {16, 32, 48, 64}) {
+        const size_t ring_v4 = ring_mib << 16, stream_v4 = ring_v4;
+        float4 *ring, *src, *dst;
+        CK(cudaMalloc(&ring, ring_v4 * 16));
+        CK(cudaMalloc(&src, stream_v4 * 16 * rounds));
+        CK(cudaMalloc(&dst, stream_v4 * 16 * rounds));
+        CK(cudaMemset(ring, 0, ring_v4 * 16));
+        CK(cudaMemset(src, 0, stream_v4 * 16 * rounds));
+        for (int split = 0; split < 2; split++) {
+            cudaEvent_t e0, e1;
+            CK(cudaEventCreate(&e0));
+            CK(cudaEventCreate(&e1));
+            CK(cudaMemset(d_ticket, 0, 8));
+            ring_by_die<<<sms * cps, 512, smem>>>(ring, ring_v4, src, dst, stream_v4, 2, split, d_die, d_ticket, (sms - n1) * cps, n1 * cps);
+            CK(cudaDeviceSynchronize());
+            CK(cudaMemset(d_ticket, 0, 8));
+            CK(cudaEventRecord(e0));
+            ring_by_die<<<sms * cps, 512, smem>>>(ring, ring_v4, src, dst, stream_v4, rounds, split, d_die, d_ticket, (sms - n1) * cps, n1 * cps);
+            CK(cudaEventRecord(e1));
+            CK(cudaDeviceSynchronize());
+            float ms = 0;
+            CK(cudaEventElapsedTime(&ms, e0, e1));
+            printf("L2 ring %2zu MiB %-28s rewritten between streams of its size: %7.3f ms; stream alone at 6.5 TB/s %6.3f ms\n", ring_mib,
+                   split ? "as two die-private halves," : "shared by both dies,", ms, (double)stream_v4 * 16 * 2 * rounds / 6.5e9);
+        }
+        CK(cudaFree(ring));
+        CK(cudaFree(src));
+        CK(cudaFree(dst));
+    }
+    CK(cudaFree(buf));
+    CK(cudaFree(out));
+    CK(cudaFree(d_die));
+    CK(cudaFree(d_ticket));
+}
+
 int main()
 {
     cudaDeviceProp prop;
@@ -264,6 +415,7 @@ int main()
             }
         }
     }
+    run_die_tests(sms);
     printf("done\n");
     return 0;
 }
