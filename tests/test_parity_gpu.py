@@ -243,6 +243,21 @@ def test_config2_full_size_reduced_sampled(hs, oracle, algo):
         assert sampled_compare(hs, oracle, d_x, v, "reduced", algo, spectra, 4000, 22) == 1
 
 
+@pytest.mark.timeout(900, method="thread")
+def test_config1_shape_full_and_reduced_output_repeated_launches(hs, oracle):
+    """configs[1]'s shape in bench's launch configuration (256 x 2^18, full + reduced output).  With both outputs the
+    warps of a CTA of the interleaved kernel (eq. 3) progress at very different speeds: the launch that once hung when
+    item completion was a running sum over the warps.  Five launches per variant, the last one compared with the oracle."""
+    d_x = W.exp_noise_torch(256, 1 << 18, 6, "cuda")
+    for v in VARIANTS:
+        plan = make_plan(hs, 1 << 18, 256, 32, v, "both", "tiled")
+        for _ in range(4):
+            plan.run(d_x)
+        plan.device_status()
+        plan.hs_destroy()
+        assert sampled_compare(hs, oracle, d_x, v, "both", "tiled", np.arange(0, 256, 37), 1500, 55) == 1
+
+
 @pytest.mark.parametrize("algo", FAMILIES)
 def test_config3_long_spectra_full_output_sampled(hs, oracle, algo):
     d_x, injected = W.config3_torch("cuda")
