@@ -465,8 +465,10 @@ __device__ __forceinline__ void add_from_x(float4 &S, const float *__restrict__ 
     S.w += t[3];
 }
 
-template <int L, int OUT, int VARIANT = HS_MAX, int HYB = 0, bool CPLX = false>
-__device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__restrict__ Ab, int64_t row, int n_first)
+// `before_slot()` is called once, before the tile's first read from the slot (after the terms taken from x when HYB = 2):
+// the warp's first tile of a spectrum waits for the group's phase-A arrivals THERE, with its x-only part already done.
+template <int L, int OUT, int VARIANT = HS_MAX, int HYB = 0, bool CPLX = false, class W>
+__device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__restrict__ Ab, int64_t row, int n_first, W &before_slot)
 {
     const int N = p.N;
     const int n = n_first + 4 * (threadIdx.x & 31);
@@ -488,10 +490,12 @@ __device__ __forceinline__ void phaseB_tile(const gr_params &p, const float *__r
     };
     emit(0);
     bool tail = false;   // levels skipped because no harmonic of theirs is in range (reduced-only output)
+    if (HYB != 2 || L <= 3) before_slot();
 #pragma unroll
     for (int l = 1; l < L; l++) {
         constexpr int kBatch = 8;
         const int lo = (1 << (l - 1)) + 1, hi = 1 << l;
+        if (HYB == 2 && L > 3 && l == 3) before_slot();                // (levels 1 and 2 came from the spectrum itself)
         if ((int64_t)lo * n_first < N) {                           // warp-uniform: the level has a harmonic in range
             if (HYB == 2 && l <= 2) {                              // sizes 2, 3, 4 are not kept: straight from the spectrum
                 if (l == 1) {
@@ -601,28 +605,29 @@ gr_kernel(const __grid_constant__ gr_params p)
         hsptx::mbar_arrive_expect_tx(&bar[buf], (uint32_t)words * 4u);
         hsptx::bulk_g2s(dyn + buf * kRaw, p.x + (int64_t)at.b * N + k0, (uint32_t)words * 4u, &bar[buf]);
     };
+    // a CTA takes the chunks rank, rank + GS, .. of a spectrum from the TOP down: the upper chunks (bins >= n_split) also
+    // emit outputs, which needs nothing but x -- work that is done before the CTA waits for the slot
+    const int c_top = rank + (p.nchunks - 1 - rank) / p.GS * p.GS;
     auto advance = [&](gr_pos at) {
-        at.c += p.GS;
-        if (at.c >= p.nchunks) {
+        at.c -= p.GS;
+        if (at.c < 0) {
             at.b += p.groups;
-            at.c = rank;
+            at.c = c_top;
         }
         return at;
     };
 
-    gr_pos cur{grp, rank};
+    gr_pos cur{grp, c_top};
     int buf = 0;
     uint32_t parity = 0u;                                                 // bit `buf`: phase of that buffer's barrier
     if (threadIdx.x == 0 && cur.b < p.B) issue(cur, 0);
 
     for (int it = 0; cur.b < p.B; it++) {
         const int b = cur.b;
-        // the slot is free once every CTA of the group has finished phase B of the previous spectrum
-        if (it > 0) {
-            if (threadIdx.x == 0) hssync::wait_count(cntB, p.GS * it, p.ctrl, p.ctrl + HS_CTRL_STATS, p.spin_limit);
-            __syncthreads();
-        }
-        // ---- phase A: this CTA's chunks of spectrum b
+        // ---- phase A: this CTA's chunks of spectrum b.  The slot is free once every CTA of the group has finished phase B
+        // of the previous spectrum: the CTA waits for that as late as possible -- after the first chunk has arrived, its
+        // sliding-maximum tables are built and (upper chunks) its outputs are emitted, just before the first store to the slot.
+        bool slot_free = it == 0;
         while (cur.b == b) {
             const gr_pos nxt = advance(cur);
             if (kRawBufs == 2 && threadIdx.x == 0 && nxt.b < p.B) issue(nxt, buf ^ 1);   // in flight while this chunk is reduced
@@ -646,8 +651,19 @@ gr_kernel(const __grid_constant__ gr_params p)
             }
             for (int w = valid + threadIdx.x; w < kRaw; w += kThreads) sm.raw[w] = 0.0f;   // zero padding (C5)
             __syncthreads();
-            phaseA_chunk<VARIANT, HMAX, HYB>(p, sm, Ab, k0);
+            constexpr bool kTabs = VARIANT == HS_MAX && HMAX >= 16;
+            if (kTabs) max_tables<HMAX>(sm);
             if (k0 >= p.n_split) emit_upper<L, OUT>(p, sm, (int64_t)b * N, k0);
+            if (!slot_free) {
+                if (threadIdx.x == 0) hssync::wait_count(cntB, p.GS * it, p.ctrl, p.ctrl + HS_CTRL_STATS, p.spin_limit);
+                slot_free = true;
+                __syncthreads();                                          // the slot is free (and the tables are complete)
+            } else if (kTabs) {
+                __syncthreads();                                          // tables complete
+            }
+            if (VARIANT == HS_MAX) max_pow2<HMAX, HYB>(p, sm, Ab, k0);
+            else dec_pow2<HMAX, HYB>(p, sm, Ab, k0);
+            other_sizes<VARIANT, HMAX, HYB>(p, sm, Ab, k0);
             __syncthreads();                                              // raw/tables/bounds are reused
             if (kRawBufs == 1 && threadIdx.x == 0 && nxt.b < p.B) issue(nxt, 0);
             cur = nxt;
@@ -656,18 +672,26 @@ gr_kernel(const __grid_constant__ gr_params p)
         if (threadIdx.x == 0) {
             s_next = 0;
             red_release_add(cntA, 1);                                     // (cumulative: ordered after the CTA's stores)
-            hssync::wait_count(cntA, p.GS * (it + 1), p.ctrl, p.ctrl + HS_CTRL_STATS, p.spin_limit);
         }
         __syncthreads();
-        // ---- phase B: the group's warps share the tiles; a CTA takes tiles rank, rank + GS, .. heavy (low n) first
+        // ---- phase B: the group's warps share the tiles; a CTA takes tiles rank, rank + GS, .. heavy (low n) first.
+        // Every A_i of the spectrum is in the slot once all CTAs of the group have arrived: each WARP waits for that inside
+        // its first tile, after the part of the tile that reads only x.
         const int64_t row = (int64_t)b * N;
+        bool arrived = false;
+        auto wait_arrivals = [&]() {
+            if (arrived) return;
+            if ((threadIdx.x & 31) == 0) hssync::wait_count(cntA, p.GS * (it + 1), p.ctrl, p.ctrl + HS_CTRL_STATS, p.spin_limit);
+            __syncwarp();
+            arrived = true;
+        };
         for (;;) {
             int j = 0;
             if ((threadIdx.x & 31) == 0) j = atomicAdd(&s_next, 1);
             j = __shfl_sync(0xffffffffu, j, 0);
             const int tile = rank + p.GS * j;
             if (tile >= p.ntiles) break;
-            phaseB_tile<L, OUT, VARIANT, HYB, CPLX>(p, Ab, row, tile * kTileB);
+            phaseB_tile<L, OUT, VARIANT, HYB, CPLX>(p, Ab, row, tile * kTileB, wait_arrivals);
         }
         __syncthreads();                                                  // every load of the slot has returned
         if (threadIdx.x == 0) red_release_add(cntB, 1);
