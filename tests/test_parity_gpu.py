@@ -269,7 +269,7 @@ def test_config3_long_spectra_full_output_sampled(hs, oracle, algo):
 @pytest.mark.parametrize("algo", FAMILIES)
 def test_scaling_shapes_short_and_long_spectra(hs, oracle, algo):
     # configs[4] scaling sweep shapes, shrunk in batch: 2^16-bin and 2^24-bin spectra, Hmax 32 and 4
-    for N, B in ((1 << 16, 64), (1 << 24, 2)):
+    for N, B in ((1 << 16, 64), (1 << 19, 40), (1 << 24, 2)):       # (2^19: the longest spectra the interleaved kernel takes)
         d_x = W.exp_noise_torch(B, N, 4, "cuda")
         for Hmax in (32, 4):
             for v in _variants_of(algo, Hmax, N):
