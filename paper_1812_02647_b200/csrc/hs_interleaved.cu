@@ -555,9 +555,10 @@ il_sched make_sched(const hs_plan *p, int64_t batch)
     // resident CTAs busy; shorter spectra need more groups in flight for that (about two items per resident CTA),
     // within the same 48 MiB.
     const int64_t slot_bytes = s.slot_words * 4;
-    int64_t R = (2 * (int64_t)kCtasPerSm * p->sm_count + s.nT - 1) / s.nT + 1;
+    // (measured with the scheduler warp: as many slots as fit 48 MiB -- 2^16 bins: 5 slots 4.3 ms, 12 slots 3.51 ms;
+    // 2^17 bins: 4 slots 4.06 ms, 6 slots 3.54 ms on 2^30 bins)
     const int64_t cap = ((int64_t)48 << 20) / slot_bytes;
-    if (R > cap) R = cap;
+    int64_t R = cap;
     if (R < kMaxRing) R = slot_bytes > ((int64_t)16 << 20) ? 2 : kMaxRing;   // (2^19-bin spectra: two 32 MiB slots)
     R = hs_knob("HS_IL_RING", (int)R);
     if (R < 2) R = 2;
