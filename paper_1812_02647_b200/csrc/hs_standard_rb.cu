@@ -117,14 +117,28 @@ template <int LV>
 __device__ __forceinline__ void emit_level(const float (&S)[32], float (&m)[32], int (&a)[32])
 {
 #pragma unroll
-    for (int r = 0; r < 32; r++) {
-        const float h = S[r] * hs_norm(LV);
+    for (int r = 0; r < 32; r += 2) {
+        // two outputs per multiply: mul.f32x2 (FMUL2) is the same IEEE fp32 product in each half
+        float h0, h1;
         if (LV == 0) {
-            m[r] = h;
-            a[r] = 0;
-        } else if (h > m[r]) {
-            m[r] = h;
-            a[r] = LV;
+            h0 = S[r], h1 = S[r + 1];
+        } else {
+            asm("{\n\t.reg .b64 a, c, d;\n\tmov.b64 a, {%2, %3};\n\tmov.b64 c, {%4, %4};\n\tmul.rn.f32x2 d, a, c;\n\tmov.b64 {%0, %1}, d;\n\t}"
+                : "=f"(h0), "=f"(h1)
+                : "f"(S[r]), "f"(S[r + 1]), "f"(hs_norm(LV)));
+        }
+        if (LV == 0) {
+            m[r] = h0, m[r + 1] = h1;
+            a[r] = 0, a[r + 1] = 0;
+        } else {
+            if (h0 > m[r]) {
+                m[r] = h0;
+                a[r] = LV;
+            }
+            if (h1 > m[r + 1]) {
+                m[r + 1] = h1;
+                a[r + 1] = LV;
+            }
         }
     }
 }
