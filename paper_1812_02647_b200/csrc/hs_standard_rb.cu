@@ -106,9 +106,15 @@ __device__ __forceinline__ void accumulate(const float *__restrict__ slot, int m
         for (int k = 0; k <= I; k++) w[k] = row[k];
     }
 #pragma unroll
-    for (int r = 0; r < 32; r++) {
-        if constexpr (I == 32) S[r] = w[cidx(r, I)];             // first harmonic of a tile: starts the running sums
-        else S[r] += w[cidx(r, I)];
+    for (int r = 0; r < 32; r += 2) {
+        if constexpr (I == 32) {                                 // first harmonic of a tile: starts the running sums
+            S[r] = w[cidx(r, I)];
+            S[r + 1] = w[cidx(r + 1, I)];
+        } else {
+            asm("{\n\t.reg .b64 a, b, d;\n\tmov.b64 a, {%0, %1};\n\tmov.b64 b, {%2, %3};\n\tadd.rn.f32x2 d, a, b;\n\tmov.b64 {%0, %1}, d;\n\t}"
+                : "+f"(S[r]), "+f"(S[r + 1])
+                : "f"(w[cidx(r, I)]), "f"(w[cidx(r + 1, I)]));
+        }
     }
 }
 
