@@ -159,11 +159,11 @@ int allh_by_out(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStre
 template <int VARIANT, int L, int OUT>
 __global__ void __launch_bounds__(kThreads)
 hs_2d_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax, uint8_t *__restrict__ amax,
-             int N, int Z)
+             int N, int Z, int zi0)
 {
     constexpr int HMAX = 1 << (L - 1), LG = L - 1;
     const int n = blockIdx.x * kThreads + threadIdx.x;
-    const int zi = blockIdx.y, Zc = (Z - 1) >> 1, z = zi - Zc;
+    const int zi = zi0 + blockIdx.y, Zc = (Z - 1) >> 1, z = zi - Zc;
     const int64_t b = blockIdx.z;
     if (n >= N) return;
     const int64_t plane = (int64_t)Z * N;
@@ -191,20 +191,68 @@ hs_2d_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__res
             level(l);
         }
     } else {
+        // Harmonic i is inside the plane iff |i z| <= (Z-1)/2 (uniform for the CTA: z is its row) and i n < N; for the warp
+        // that holds bins n_lo .. n_lo + 31 no harmonic beyond imax has any term: those harmonics, and the levels made of
+        // them only, are skipped warp-uniformly (most rows of a plane have |z| > (Z-1)/4 and no harmonic but the first).
+        const int n_lo = n & ~31;
+        int imax = HMAX;
+        if (z != 0) imax = min(imax, Zc / (z < 0 ? -z : z));
+        if (n_lo > 0) imax = min(imax, (N - 1) / n_lo);
+        bool tail = false;   // levels skipped because none of their harmonics is in range (reduced-only output)
 #pragma unroll
         for (int l = 1; l < L; l++) {
-#pragma unroll
-            for (int i = (1 << (l - 1)) + 1; i <= (1 << l); i++) {
-                const int k = i * n, row = i * z + Zc;
-                if (k < N && row >= 0 && row < Z) S += __ldg(xb + (int64_t)row * N + k);
+            const int lo = (1 << (l - 1)) + 1, hi = 1 << l;
+            if (lo <= imax) {
+                for (int i = lo; i <= hi && i <= imax; i++) {
+                    const int k = i * n;
+                    if (k < N) S += __ldg(xb + (int64_t)(i * z + Zc) * N + k);
+                }
+                level(l);
+            } else if ((OUT & 3) != HS_OUT_REDUCED) {
+                level(l);
+            } else {
+                tail = true;
             }
-            level(l);
         }
+        // With S unchanged over the skipped levels h_l = S c_l is monotone in l: testing the last level alone is enough.
+        if ((OUT & 3) == HS_OUT_REDUCED && tail) level(L - 1);
     }
     if (OUT & HS_OUT_REDUCED) {
         const int64_t o = b * plane + (int64_t)zi * N + n;
         hsptx::st_cs(vmax + o, e.m);
         hsptx::st_cs(amax + o, (uint8_t)e.a);
+    }
+}
+
+// 2-D freq-bin, rows whose drift is so large that no harmonic but the first is inside the plane (|2 z| > (Z-1)/2: half of
+// the rows): S_H = x for every H, a pure stream.  Four bins per thread; h_l = x c_l is monotone in l, so the first level
+// wins for x >= 0 (ties included, C8) and the last one for x < 0.  Rows [0, rows_lo) and [Z - rows_lo, Z) of each plane.
+template <int L, int OUT>
+__global__ void __launch_bounds__(kThreads)
+hs_2d_outer_rows_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
+                        uint8_t *__restrict__ amax, int N, int Z, int rows_lo)
+{
+    const int n = 4 * (blockIdx.x * kThreads + threadIdx.x);
+    if (n >= N) return;
+    const int r = blockIdx.y, zi = r < rows_lo ? r : Z - 2 * rows_lo + r;
+    const int64_t plane = (int64_t)Z * N, o = (int64_t)blockIdx.z * plane + (int64_t)zi * N + n;
+    const float4 v = __ldg(reinterpret_cast<const float4 *>(x + o));
+    if (OUT & HS_OUT_FULL) {
+        float *p0 = sums + ((int64_t)blockIdx.z * L) * plane + (int64_t)zi * N + n;
+#pragma unroll
+        for (int l = 0; l < L; l++) {
+            const float c = hs_norm(l);
+            hsptx::st_cs(reinterpret_cast<float4 *>(p0 + (int64_t)l * plane),
+                         l == 0 ? v : make_float4(v.x * c, v.y * c, v.z * c, v.w * c));
+        }
+    }
+    if (OUT & HS_OUT_REDUCED) {
+        const float c = hs_norm(L - 1);
+        hsptx::st_cs(reinterpret_cast<float4 *>(vmax + o), make_float4(v.x < 0.f ? v.x * c : v.x, v.y < 0.f ? v.y * c : v.y,
+                                                                       v.z < 0.f ? v.z * c : v.z, v.w < 0.f ? v.w * c : v.w));
+        hsptx::st_cs(reinterpret_cast<uint32_t *>(amax + o),
+                     (v.x < 0.f ? (uint32_t)(L - 1) : 0u) | (v.y < 0.f ? (uint32_t)(L - 1) << 8 : 0u) |
+                         (v.z < 0.f ? (uint32_t)(L - 1) << 16 : 0u) | (v.w < 0.f ? (uint32_t)(L - 1) << 24 : 0u));
     }
 }
 
@@ -217,10 +265,20 @@ int launch_2d(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream
     for (int64_t b0 = 0; b0 < batch; b0 += 65535) {
         const unsigned nb = (unsigned)(batch - b0 < 65535 ? batch - b0 : 65535);
         const int64_t off = b0 * plane;
-        hs_2d_kernel<VARIANT, L, OUT><<<dim3(tiles, (unsigned)Z, nb), kThreads, 0, stream>>>(
+        // freq-bin, L > 1: the rows with |2 z| > (Z-1)/2 have no harmonic but the first inside the plane: streamed (N % 4 == 0)
+        const int Zc = (Z - 1) / 2;
+        const int rows_lo = (VARIANT == HS_FREQBIN && L > 1) ? Zc - Zc / 2 : 0;   // rows zi < rows_lo <=> z < -(Zc / 2)
+        hs_2d_kernel<VARIANT, L, OUT><<<dim3(tiles, (unsigned)(Z - 2 * rows_lo), nb), kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
-            buf.amax ? buf.amax + off : nullptr, N, Z);
+            buf.amax ? buf.amax + off : nullptr, N, Z, rows_lo);
         HS_CUDA_OK(cudaGetLastError());
+        if (rows_lo > 0) {
+            const unsigned t4 = (unsigned)((N / 4 + kThreads - 1) / kThreads);
+            hs_2d_outer_rows_kernel<L, OUT><<<dim3(t4, (unsigned)(2 * rows_lo), nb), kThreads, 0, stream>>>(
+                buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
+                buf.amax ? buf.amax + off : nullptr, N, Z, rows_lo);
+            HS_CUDA_OK(cudaGetLastError());
+        }
     }
     return HS_OK;
 }
