@@ -10,6 +10,17 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    config.addinivalue_line("markers", "timeout: per-test time limit (pytest-timeout; ignored if the plugin is absent)")
+
+
+def pytest_collection_modifyitems(config, items):
+    """A GPU test that does not come back (a persistent kernel that hangs) must end the run, not block the box: every
+    GPU test gets a 15-minute limit enforced from a watchdog thread (pytest-timeout, if installed)."""
+    if not config.pluginmanager.hasplugin("timeout"):
+        return
+    for item in items:
+        if "gpu" in item.keywords and item.get_closest_marker("timeout") is None:
+            item.add_marker(pytest.mark.timeout(900, method="thread"))
 
 
 @pytest.fixture(scope="session")
