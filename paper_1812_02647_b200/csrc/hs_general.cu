@@ -65,6 +65,21 @@ hs_allh_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__r
     if (live) e.level(0, S, 1.0f, plane0, N);
     if (JDBG && live) jplane0[0] = 0;
     for (int H = 2; H <= Hmax; H++) {
+        // eqs. 2-4, reduced output only: once harmonic H is out of range for the whole warp so is every later one and S
+        // stays what it is.  h = S c_H is then monotone in H, so of the remaining levels only the first (in the dyadic mode
+        // it may be the first to see the last in-range harmonics) and the last can change the maximum.
+        if (VARIANT != HS_STANDARD && (OUT & 3) == HS_OUT_REDUCED && !JDBG && (int64_t)H * n_lo + J0 >= N) {
+            int Hf = H;
+            if (dyadic) {
+                Hf = 1;
+                while (Hf < H) Hf <<= 1;                                // the first level at or after H
+            }
+            if (live && Hf <= Hmax) {
+                e.level(dyadic ? 31 - __clz(Hf) : Hf - 1, S, norm_any(Hf), plane0, N);
+                if (Hf != Hmax) e.level(L - 1, S, norm_any(Hmax), plane0, N);
+            }
+            break;
+        }
         const float cn = norm_any(H);
         if (VARIANT == HS_STANDARD) {
             // eq. 1 is not cumulative over consecutive H: every level from scratch.  Index of term i: nearest(n i / H),
