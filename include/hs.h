@@ -48,8 +48,10 @@ enum hs_status {
     HS_ERR_UNSUPPORTED = 4,  /* no CUDA device of compute capability 10.x is current                    */
     HS_ERR_WORKSPACE = 5,    /* the chosen algorithm needs a workspace that was not set or is too small */
     HS_ERR_CUDA = 6,         /* a CUDA runtime call or kernel launch failed                             */
-    HS_ERR_DEVICE_TIMEOUT = 7 /* hs_plan_device_status: a kernel of the last execute gave up waiting for another
+    HS_ERR_DEVICE_TIMEOUT = 7, /* hs_plan_device_status: a kernel of the last execute gave up waiting for another
                                  thread block (its outputs are then not valid)                          */
+    HS_ERR_SCRATCH_LIMIT = 8  /* hs_execute_static: one spectrum's per-harmonic arrays do not fit the library's
+                                 built-in scratch array (HS_STATIC_SCRATCH_BYTES)                       */
 };
 /* Kernel family.  HS_ALGO_AUTO picks the fastest one that is valid for the plan. */
 enum hs_algo {
@@ -211,6 +213,43 @@ typedef struct hs_candidate {
 } hs_candidate;
 int hs_execute_candidates(const hs_plan *plan, const float *d_x, float threshold, hs_candidate *d_cand,
                           int64_t capacity, unsigned long long *d_count, void *stream);
+
+/*
+ * hs_execute_static — eqs. 2 and 3 for callers that have no way to get device scratch memory.
+ *
+ * Every other execute call of this library leaves allocation to the caller: a kernel family that needs scratch wants
+ * a workspace from hs_plan_set_workspace.  Some callers cannot provide one.  A real-time search back end typically
+ * reserves all of its device memory when the observation starts and bans cudaMalloc / cudaFree inside the observing
+ * loop (both synchronise the whole device, and an allocation can still fail hours into a run); a plug-in that a host
+ * application hands input and output buffers to owns no allocator at all; and a process whose framework has claimed
+ * the device's memory up front gets an out-of-memory error from a raw cudaMalloc.  For those callers this entry
+ * point runs the two-phase kernels (the HS_ALGO_TWOPHASE family: phase 1 writes the per-harmonic arrays A_i of a
+ * group of spectra, phase 2 sums them) with the arrays kept in a fixed array that is part of the library image:
+ * HS_STATIC_SCRATCH_BYTES (32 MiB) of device memory, held by every GPU on which the library's code is loaded, from
+ * then until the process exits.  The call allocates nothing: no cudaMalloc, no cudaFree, no library routine that does.
+ *
+ *   plan     from hs_plan_create with variant HS_MAX or HS_FREQBIN (anything else, and plans of hs_plan_create_ex
+ *            with non-default options or of hs_plan_create_2d: HS_ERR_INVALID_ARG).  Any Hmax, any out_mode, any
+ *            batch: the batch is processed in groups of as many spectra as fit the array.  The plan's own algorithm
+ *            choice and workspace are ignored.
+ *   limit    one spectrum's arrays (about 3.06 * nbins floats at Hmax = 32, 1.08 * nbins at Hmax = 4) must fit:
+ *            about 2.7 million bins at Hmax = 32 (2^21 fits, 2^22 does not).  Longer spectra fail with HS_ERR_SCRATCH_LIMIT before anything is
+ *            enqueued; hs_static_scratch_bytes() returns the size of the array.
+ *   buffers  d_x, d_sums, d_max, d_argmax: DEVICE pointers owned by the caller, layouts, NULL and alignment rules and
+ *            asynchrony exactly as hs_execute; the outputs are those of hs_execute on a HS_ALGO_TWOPHASE plan.
+ *
+ * First call on a device: the library looks up the device address of its array (once per device, with that device
+ * current) before it launches.  Make that first call outside any stream capture.
+ * Sharing: there is ONE array per device, shared by every plan, thread and stream, and it keeps whatever the previous
+ * call left in it.  Nothing in it has to start at zero (phase 1 writes every word that phase 2 reads, before it reads
+ * it), so a call never sees another call's data as long as calls do not overlap on the GPU; two calls that can run at
+ * the same time (different streams with no dependency between them) race on the array and both produce garbage.
+ * Order them with events, or use hs_execute with one caller-owned workspace per plan.
+ */
+#define HS_STATIC_SCRATCH_BYTES (32u << 20)
+int hs_execute_static(const hs_plan *plan, const float *d_x, float *d_sums, float *d_max, uint8_t *d_argmax,
+                      void *stream);
+size_t hs_static_scratch_bytes(void);    /* HS_STATIC_SCRATCH_BYTES of the library that is loaded                 */
 
 /*
  * hs_debug_greedy_paths — test-only: Greedy's drift j after each level, d_j[batch][L][nbins] uint8 (DEVICE),

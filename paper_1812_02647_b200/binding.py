@@ -22,6 +22,7 @@ LEVELS = {"dyadic": HS_LEVELS_DYADIC, "all": HS_LEVELS_ALL}
 WINDOWS = {"c2": HS_WINDOW_C2, "printed": HS_WINDOW_PRINTED}
 (HS_OK, HS_ERR_INVALID_ARG, HS_ERR_NULL_POINTER, HS_ERR_MISALIGNED, HS_ERR_UNSUPPORTED, HS_ERR_WORKSPACE, HS_ERR_CUDA,
  HS_ERR_DEVICE_TIMEOUT) = range(8)
+HS_ERR_SCRATCH_LIMIT = 8
 VARIANTS = {"standard": HS_STANDARD, "max": HS_MAX, "freqbin": HS_FREQBIN, "greedy": HS_GREEDY}
 OUT_MODES = {"full": HS_OUT_FULL, "reduced": HS_OUT_REDUCED, "both": HS_OUT_BOTH}
 ALGOS = {"auto": HS_ALGO_AUTO, "direct": HS_ALGO_DIRECT, "tiled": HS_ALGO_TILED, "twophase": HS_ALGO_TWOPHASE,
@@ -55,6 +56,8 @@ _SIGS = {
     "hs_plan_set_host_staging": ([_p, _p, _sz, _i64], _int),
     "hs_debug_greedy_paths": ([_p, _p, _p, _p], _int),
     "hs_execute_candidates": ([_p, _p, ctypes.c_float, _p, _i64, _p, _p], _int),
+    "hs_execute_static": ([_p, _p, _p, _p, _p, _p], _int),
+    "hs_static_scratch_bytes": ([], _sz),
 }
 for _name, (_args, _res) in _SIGS.items():
     _f = getattr(lib, _name)
@@ -162,6 +165,14 @@ class Plan:
     def hs_execute(self, d_x, d_sums=None, d_max=None, d_argmax=None, stream=None):
         _check(lib.hs_execute(self.handle, _ptr(d_x), _ptr(d_sums), _ptr(d_max), _ptr(d_argmax), _stream(stream)),
                "hs_execute")
+
+    def hs_execute_static(self, d_x, d_sums=None, d_max=None, d_argmax=None, stream=None):
+        """eqs. 2-3 through the library's built-in scratch array, for callers that cannot allocate device memory (see
+        include/hs.h): the caller passes inputs and outputs only; no workspace is set, taken or allocated.  Raises
+        HsError(HS_ERR_SCRATCH_LIMIT) when one spectrum's arrays exceed hs_static_scratch_bytes().  Calls share the one
+        array: do not let two of them overlap on the GPU."""
+        _check(lib.hs_execute_static(self.handle, _ptr(d_x), _ptr(d_sums), _ptr(d_max), _ptr(d_argmax), _stream(stream)),
+               "hs_execute_static")
 
     def hs_execute_complex(self, d_F, scale, d_sums=None, d_max=None, d_argmax=None, stream=None):
         """d_F: complex64 (or float32 [..., 2]) CUDA tensor [batch][nbins]; x = |F|^2 * scale - 1 is formed inside the kernels."""

@@ -118,6 +118,8 @@ const char *hs_error_string(int code)
         case HS_ERR_WORKSPACE: return "workspace or staging buffer missing or too small";
         case HS_ERR_CUDA: return "CUDA runtime call or kernel launch failed";
         case HS_ERR_DEVICE_TIMEOUT: return "a kernel gave up waiting for another thread block: outputs are not valid";
+        case HS_ERR_SCRATCH_LIMIT:
+            return "one spectrum's per-harmonic arrays exceed the library's built-in scratch array (HS_STATIC_SCRATCH_BYTES)";
         default: return "unknown hs_status code";
     }
 }

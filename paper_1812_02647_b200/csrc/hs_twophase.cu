@@ -17,6 +17,8 @@
 // the blocks of size 2j, 4j, .. <= Hmax are unions of aligned pairs, so they come from a shuffle-xor pyramid over
 // neighbouring lanes (M_2j(n) = max(M_j(2n), M_j(2n+1))).  A chunk owns the super-blocks (size j*K_j, K_j the largest
 // power of two with j*K_j <= Hmax) that START inside it, and reads a 32-word halo for those that run past its end.
+#include <mutex>
+
 #include "hs_internal.cuh"
 #include "hs_ptx.cuh"
 
@@ -432,4 +434,133 @@ int hs_twophase_launch(const hs_plan *p, const hs_buffers &buf, int64_t batch, v
     if (!ws) HS_FAIL(HS_ERR_WORKSPACE);
     if (p->variant == HS_FREQBIN) return by_hmax<HS_FREQBIN>(p, buf, batch, ws, stream);
     return by_hmax<HS_MAX>(p, buf, batch, ws, stream);
+}
+
+// ------------------------------------------------------------------------ hs_execute_static: scratch inside the library
+// For callers that cannot hand the library a workspace because they cannot allocate device memory at all (a search loop
+// that has banned cudaMalloc after start-up, a plug-in that is only ever given input and output buffers, a process whose
+// framework holds all of the device's memory): the same two kernels, their per-harmonic arrays kept in an array that is
+// part of this module's image.  See include/hs.h for the contract.  Nothing above this line is touched by it.
+
+namespace {
+
+// The scratch itself.  Device code may use the name; in HOST code `g_static_scratch` is only a handle for the runtime's
+// symbol table (its host address is NOT where the data lives), so the launcher below asks the runtime for the device
+// address and hands that to the kernels.  Each device has its own copy, allocated when this module is loaded there.
+static __device__ __align__(256) unsigned char g_static_scratch[HS_STATIC_SCRATCH_BYTES];
+
+constexpr int kMaxCachedDevices = 64;
+std::mutex g_static_mutex;
+void *g_static_addr[kMaxCachedDevices];   // device address of g_static_scratch per device ordinal, nullptr = not looked up
+
+// Device address of the array on device `dev`, which must be current.  The first call per device does the look-up
+// (cudaGetSymbolAddress loads the module if need be: keep it out of stream capture); later calls read the cache.
+int static_scratch_address(int dev, void **out)
+{
+    const bool cached = dev >= 0 && dev < kMaxCachedDevices;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (cached && g_static_addr[dev]) {
+        *out = g_static_addr[dev];
+        return HS_OK;
+    }
+    void *ptr = nullptr;
+    HS_CUDA_OK(cudaGetSymbolAddress(&ptr, g_static_scratch));
+    if (!ptr || (reinterpret_cast<uintptr_t>(ptr) % 256) != 0) HS_FAIL(HS_ERR_CUDA);
+    if (cached) g_static_addr[dev] = ptr;
+    *out = ptr;
+    return HS_OK;
+}
+
+// launch<> above with the slot ring at `A` holding R spectra (instead of a caller's workspace sized by make_sched)
+template <int VARIANT, int HMAX, int OUT>
+int launch_in(const hs_plan *p, const hs_buffers &buf, float *A, int R, cudaStream_t stream)
+{
+    const int N = (int)p->nbins;
+    tp_params prm{};
+    prm.x = buf.x;
+    prm.A = A;
+    prm.sums = buf.sums;
+    prm.vmax = buf.vmax;
+    prm.amax = buf.amax;
+    prm.sink = buf.sink;
+    prm.lay = make_layout(N, p->Hmax);
+    prm.N = N;
+    prm.B = (int)p->batch;
+    prm.nchunks = p->Hmax > 1 ? (N + kChunk - 1) / kChunk : 0;
+    prm.ntiles = (N + kTile2 - 1) / kTile2;
+    prm.R = R;
+    constexpr int L = HMAX == 1 ? 1 : HMAX == 2 ? 2 : HMAX == 4 ? 3 : HMAX == 8 ? 4 : HMAX == 16 ? 5 : 6;
+    // groups of R spectra in stream order: phase 2 of a group has read the slots before phase 1 of the next refills them
+    for (int64_t b0 = 0; b0 < p->batch; b0 += R) {
+        const int nb = (int)((p->batch - b0 < R) ? p->batch - b0 : R);
+        if (prm.nchunks > 0) {
+            tp_phase1_kernel<VARIANT, HMAX><<<dim3((unsigned)prm.nchunks, (unsigned)nb), kThreads, 0, stream>>>(prm, (int)b0);
+            HS_CUDA_OK(cudaGetLastError());
+        }
+        tp_phase2_kernel<L, OUT><<<dim3((unsigned)prm.ntiles, (unsigned)nb), kThreads, 0, stream>>>(prm, (int)b0);
+        HS_CUDA_OK(cudaGetLastError());
+    }
+    return HS_OK;
+}
+
+template <int VARIANT, int HMAX>
+int in_by_out(const hs_plan *p, const hs_buffers &buf, float *A, int R, cudaStream_t stream)
+{
+    switch (p->out_mode) {
+        case HS_OUT_FULL: return launch_in<VARIANT, HMAX, HS_OUT_FULL>(p, buf, A, R, stream);
+        case HS_OUT_REDUCED: return launch_in<VARIANT, HMAX, HS_OUT_REDUCED>(p, buf, A, R, stream);
+        default: return launch_in<VARIANT, HMAX, HS_OUT_BOTH>(p, buf, A, R, stream);
+    }
+}
+
+template <int VARIANT>
+int in_by_hmax(const hs_plan *p, const hs_buffers &buf, float *A, int R, cudaStream_t stream)
+{
+    switch (p->Hmax) {
+        case 1: return in_by_out<VARIANT, 1>(p, buf, A, R, stream);
+        case 2: return in_by_out<VARIANT, 2>(p, buf, A, R, stream);
+        case 4: return in_by_out<VARIANT, 4>(p, buf, A, R, stream);
+        case 8: return in_by_out<VARIANT, 8>(p, buf, A, R, stream);
+        case 16: return in_by_out<VARIANT, 16>(p, buf, A, R, stream);
+        default: return in_by_out<VARIANT, 32>(p, buf, A, R, stream);
+    }
+}
+
+bool aligned16(const void *q) { return (reinterpret_cast<uintptr_t>(q) % 16) == 0; }
+
+}  // namespace
+
+extern "C" size_t hs_static_scratch_bytes(void) { return (size_t)HS_STATIC_SCRATCH_BYTES; }
+
+extern "C" int hs_execute_static(const hs_plan *p, const float *d_x, float *d_sums, float *d_max, uint8_t *d_argmax,
+                                 void *stream)
+{
+    if (!p) HS_FAIL(HS_ERR_NULL_POINTER);
+    if ((p->variant != HS_MAX && p->variant != HS_FREQBIN) || p->nz != 1 || p->levels_mode != HS_LEVELS_DYADIC ||
+        p->window != HS_WINDOW_C2)
+        HS_FAIL(HS_ERR_INVALID_ARG);
+    // how many spectra's arrays the built-in array holds; a spectrum that does not fit on its own is refused here,
+    // before anything is enqueued (Hmax = 1 has no arrays: one group)
+    const int64_t slot_bytes = make_layout((int)p->nbins, p->Hmax).slot_words * 4;
+    int64_t R = slot_bytes > 0 ? (int64_t)HS_STATIC_SCRATCH_BYTES / slot_bytes : p->batch;
+    if (R < 1) HS_FAIL(HS_ERR_SCRATCH_LIMIT);
+    if (R > 65535) R = 65535;                                           // gridDim.y
+    if (R > p->batch) R = p->batch;
+    if (!d_x) HS_FAIL(HS_ERR_NULL_POINTER);
+    if ((p->out_mode & HS_OUT_FULL) && !d_sums) HS_FAIL(HS_ERR_NULL_POINTER);
+    if ((p->out_mode & HS_OUT_REDUCED) && (!d_max || !d_argmax)) HS_FAIL(HS_ERR_NULL_POINTER);
+    if (!aligned16(d_x) || !aligned16(d_sums) || !aligned16(d_max) || !aligned16(d_argmax)) HS_FAIL(HS_ERR_MISALIGNED);
+    int dev = -1;
+    HS_CUDA_OK(cudaGetDevice(&dev));
+    if (dev != p->device) HS_FAIL(HS_ERR_INVALID_ARG);
+    void *scratch = nullptr;
+    const int rc = static_scratch_address(dev, &scratch);
+    if (rc != HS_OK) return rc;
+    p->n_last_ctrl = 0;                                                 // (no control block: hs_plan_device_status -> HS_OK)
+    hs_buffers buf{d_x, (p->out_mode & HS_OUT_FULL) ? d_sums : nullptr, (p->out_mode & HS_OUT_REDUCED) ? d_max : nullptr,
+                   (p->out_mode & HS_OUT_REDUCED) ? d_argmax : nullptr, nullptr, {}, false, 0.0f};
+    float *A = static_cast<float *>(scratch);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (p->variant == HS_FREQBIN) return in_by_hmax<HS_FREQBIN>(p, buf, A, (int)R, s);
+    return in_by_hmax<HS_MAX>(p, buf, A, (int)R, s);
 }
