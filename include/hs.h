@@ -157,7 +157,7 @@ int hs_last_error(void);                 /* code of the last failed call on this
 const char *hs_error_string(int code);   /* static string, never NULL                                            */
 const char *hs_version(void);            /* static string                                                        */
 
-int hs_plan_levels(const hs_plan *plan);                 /* L = log2(Hmax)+1, or -1 if plan is NULL               */
+int hs_plan_levels(const hs_plan *plan);                 /* L = log2(Hmax)+1 (HS_LEVELS_ALL plans: Hmax); -1 if NULL */
 int hs_plan_set_algo(hs_plan *plan, int algo);           /* enum hs_algo; resets the workspace requirement       */
 int hs_plan_algo(const hs_plan *plan);                   /* the resolved family (never HS_ALGO_AUTO), -1 if NULL */
 size_t hs_plan_workspace_bytes(const hs_plan *plan);     /* device scratch the resolved algorithm needs (0 = none) */
@@ -209,7 +209,7 @@ typedef struct hs_candidate {
     int32_t spectrum; /* b */
     int32_t bin;      /* n */
     float value;      /* m(b, n) */
-    int32_t level;    /* a(b, n): level index l = log2 H of the best level, smallest on ties */
+    int32_t level;    /* a(b, n): level index of the best level, smallest on ties: l = log2 H (HS_LEVELS_ALL plans: H - 1) */
 } hs_candidate;
 int hs_execute_candidates(const hs_plan *plan, const float *d_x, float threshold, hs_candidate *d_cand,
                           int64_t capacity, unsigned long long *d_count, void *stream);

@@ -271,12 +271,7 @@ int hs_plan_launches(const hs_plan *p)
 {
     if (!p) return -1;
     if (p->algo == HS_ALGO_TILED) return hs_tiled_launches(p, p->batch);
-    if (p->algo == HS_ALGO_GENERAL) {
-        if (hs_general_workspace_bytes(p)) return 2;
-        // (the 2-D freq-bin sum streams its outer rows with a second kernel: hs_general.cu)
-        const int per_slab = (p->nz >= 5 && p->variant == HS_FREQBIN && p->L > 1) ? 2 : 1;
-        return per_slab * (int)((p->batch + 65534) / 65535);
-    }
+    if (p->algo == HS_ALGO_GENERAL) return hs_general_launches(p);   // (counted next to the launcher: hs_general.cu)
     const int64_t tiles = (p->nbins + 255) / 256;
     const int64_t max_spectra = ((int64_t)1 << 30) / tiles;
     return (int)((p->batch + max_spectra - 1) / max_spectra);

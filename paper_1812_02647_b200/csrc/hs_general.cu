@@ -14,8 +14,19 @@ namespace {
 
 constexpr int kThreads = 256;
 
-// h_H = S_H / sqrt(H) for any integer H: fp32 multiply by the correctly rounded fp32 reciprocal root (C7 generalised)
-__device__ __forceinline__ float norm_any(int H) { return 1.0f / sqrtf((float)H); }
+// h_H = S_H / sqrt(H) for any integer H: fp32 multiply by the correctly rounded fp32 reciprocal root (C7 generalised),
+// c_H = fp32(1 / sqrt(H)) evaluated in double: the nine-digit literals below round to exactly those values.  (The fp32
+// expression 1.0f / sqrtf((float)H) rounds twice and is one ulp off for H = 6, 7, 17, 18, 21, 24, 28, 34, 39, 55, 58, 61.)
+__constant__ float c_norm_any[64] = {
+    1.0f, 0.707106769f, 0.577350259f, 0.5f, 0.44721359f, 0.408248305f, 0.377964467f, 0.353553385f,
+    0.333333343f, 0.316227764f, 0.301511347f, 0.288675129f, 0.277350098f, 0.267261237f, 0.258198887f, 0.25f,
+    0.242535621f, 0.235702261f, 0.22941573f, 0.223606795f, 0.218217894f, 0.213200718f, 0.208514407f, 0.204124153f,
+    0.200000003f, 0.196116135f, 0.192450091f, 0.188982233f, 0.185695335f, 0.182574183f, 0.179605305f, 0.176776692f,
+    0.17407766f, 0.171498582f, 0.169030845f, 0.166666672f, 0.164398983f, 0.162221417f, 0.160128146f, 0.158113882f,
+    0.156173766f, 0.154303357f, 0.152498573f, 0.150755674f, 0.149071202f, 0.147441953f, 0.145864993f, 0.144337565f,
+    0.142857149f, 0.141421363f, 0.140028015f, 0.138675049f, 0.137360558f, 0.136082768f, 0.134839967f, 0.133630618f,
+    0.132453233f, 0.13130644f, 0.130188912f, 0.129099444f, 0.128036886f, 0.127000123f, 0.125988156f, 0.125f};
+__device__ __forceinline__ float norm_any(int H) { return c_norm_any[H - 1]; }
 
 // running reduced output over the levels l = H - 1 (C8: a level replaces the maximum only if strictly greater)
 template <int OUT>
@@ -271,6 +282,14 @@ hs_2d_outer_rows_kernel(const float *__restrict__ x, float *__restrict__ sums, f
     }
 }
 
+// rows at each edge of the plane that the streaming kernel takes (0: none, one launch per slab); also what
+// hs_general_launches counts with
+int outer_rows(int Z, int variant, int L)
+{
+    const int Zc = (Z - 1) / 2;
+    return (variant == HS_FREQBIN && L > 1) ? Zc - Zc / 2 : 0;
+}
+
 template <int VARIANT, int L, int OUT>
 int launch_2d(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream_t stream)
 {
@@ -281,8 +300,7 @@ int launch_2d(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStream
         const unsigned nb = (unsigned)(batch - b0 < 65535 ? batch - b0 : 65535);
         const int64_t off = b0 * plane;
         // freq-bin, L > 1: the rows with |2 z| > (Z-1)/2 have no harmonic but the first inside the plane: streamed (N % 4 == 0)
-        const int Zc = (Z - 1) / 2;
-        const int rows_lo = (VARIANT == HS_FREQBIN && L > 1) ? Zc - Zc / 2 : 0;   // rows zi < rows_lo <=> z < -(Zc / 2)
+        const int rows_lo = outer_rows(Z, VARIANT, L);                            // rows zi < rows_lo <=> z < -(Zc / 2)
         hs_2d_kernel<VARIANT, L, OUT><<<dim3(tiles, (unsigned)(Z - 2 * rows_lo), nb), kThreads, 0, stream>>>(
             buf.x + off, buf.sums ? buf.sums + off * L : nullptr, buf.vmax ? buf.vmax + off : nullptr,
             buf.amax ? buf.amax + off : nullptr, N, Z, rows_lo);
@@ -328,6 +346,14 @@ int d2_by_level(const hs_plan *p, const hs_buffers &buf, int64_t batch, cudaStre
 size_t hs_general_workspace_bytes(const hs_plan *p)
 {
     return (p->nz > 1 && hs_standard_rb_supported(p)) ? hs_standard_rb_workspace_bytes(p) : 0;
+}
+
+// kernel launches (memset nodes included) of one hs_launch_general over the plan's batch
+int hs_general_launches(const hs_plan *p)
+{
+    if (hs_general_workspace_bytes(p)) return 2;                        // rb_kernel: memset node + kernel
+    const int per_slab = (p->nz > 1 && outer_rows((int)p->nz, p->variant, p->L) > 0) ? 2 : 1;
+    return per_slab * (int)((p->batch + 65534) / 65535);
 }
 
 int hs_launch_general(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream)

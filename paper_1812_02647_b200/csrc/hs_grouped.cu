@@ -19,7 +19,7 @@
 // chunk of a spectrum is an upper one whose TMA wait, tables and upper-half outputs come before the wait for "slot free"
 // (which sits just before the first store to the slot), and each warp waits for the phase-A arrivals inside its first
 // phase-B tile, after the terms it takes from x itself (6.69 -> 5.94 ms on 4096 x 2^18).
-// groups x slot is sized to ~56 MB, so the A traffic (3.06 N words written, 3.06 N read per spectrum) stays in L2 and
+// groups x slot is sized to the L2 budget (make_sched: 18 groups of 32 CTAs = 37 MB of slots at 2^18 bins, Hmax 32), so the A traffic (3.06 N words written, 3.06 N read per spectrum) stays in L2 and
 // HBM sees x once and the outputs once: 9 B/bin in reduced mode.  No CTA ever waits for a CTA outside its group, the
 // schedule is static (no work queue), and a waiting CTA shares its SM with a CTA of another group.
 //

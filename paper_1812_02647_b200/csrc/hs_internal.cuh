@@ -102,6 +102,7 @@ struct hs_buffers {
 int hs_launch_direct(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
 int hs_launch_general(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);   // hs_general.cu
 size_t hs_general_workspace_bytes(const hs_plan *p);
+int hs_general_launches(const hs_plan *p);
 int hs_launch_tiled(const hs_plan *p, const hs_buffers &buf, int64_t batch, void *ws, cudaStream_t stream);
 size_t hs_tiled_workspace_bytes(const hs_plan *p, int64_t batch);
 int hs_tiled_launches(const hs_plan *p, int64_t batch);

@@ -82,18 +82,23 @@ def test_eq2_window_as_printed(hs, ext):
         x, _ = W.comb_batch_numpy(2, list(range(B)), N, 1.0, 5.0, max(6.0, N / 40), 0.10) if N >= 256 else \
             ((np.random.default_rng(43).standard_exponential((B, N)) - 1).astype(np.float32), None)
         d_x = torch.from_numpy(x).cuda()
-        plan = hs.hs_plan_create_ex(N, B, Hmax, "max", "both", levels, "printed")
-        sums, vmax, amax = plan.run(d_x)
-        torch.cuda.synchronize()
         ref = ext.harmonic_sum_all(x, Hmax, "max", "printed")
         if levels == "dyadic":                                   # the dyadic levels of the all-H oracle
             pick = [h - 1 for h in (1, 2, 4, 8, 16, 32, 64) if h <= Hmax]
             ref_sums = ref["sums"][:, pick]
             best, second, gap, m = argmax_from_levels(np.moveaxis(ref_sums, 1, -1))
             ref = {"sums": ref_sums, "max": m, "argmax": best, "second": second, "gap": gap}
-        compare(plan, (sums, vmax, amax), ref, f"printed window N={N} Hmax={Hmax} {levels}", printed=True)
         shifted = np.concatenate([x[:, 1:], np.zeros((B, 1), np.float32)], axis=1)          # h_1(n) = x(n + 1)
-        np.testing.assert_array_equal(sums[:, 0].cpu().numpy(), shifted)
+        # ("reduced" alone is the only mode in which the kernel stops at the first harmonic that is out of range for the warp
+        # and emits the first and the last remaining level only)
+        for out_mode in ("both", "reduced", "full"):
+            plan = hs.hs_plan_create_ex(N, B, Hmax, "max", out_mode, levels, "printed")
+            sums, vmax, amax = plan.run(d_x)
+            torch.cuda.synchronize()
+            compare(plan, (sums, vmax, amax), ref, f"printed window N={N} Hmax={Hmax} {levels} {out_mode}", printed=True)
+            if sums is not None:
+                np.testing.assert_array_equal(sums[:, 0].cpu().numpy(), shifted)
+            plan.hs_destroy()
     with pytest.raises(hs.HsError) as e:
         hs.hs_plan_create_ex(4096, 1, 32, "greedy", "full", "dyadic", "printed")
     assert e.value.code == hs.HS_ERR_INVALID_ARG
@@ -116,6 +121,29 @@ def test_general_plans_reject_other_families_and_bad_arguments(hs):
         assert e.value.code == hs.HS_ERR_INVALID_ARG
     d = hs.hs_plan_create_ex(4096, 1, 32, "max", "full", "dyadic", "c2")          # the plain plan: not general
     assert d.algo != hs.HS_ALGO_GENERAL
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_candidates_on_every_integer_H_plans(hs, ext, variant):
+    """hs_execute_candidates on HS_LEVELS_ALL plans (level = H - 1) and on the printed window: the records are the bins
+    whose reduced maximum, as the all-H oracle gives it, exceeds the threshold."""
+    from parity import check_candidates
+    for N, B, Hmax, window in ((20000, 3, 48, "c2"), (4100, 2, 64, "c2"), (1 << 15, 2, 17, "printed")):
+        if window == "printed" and variant != "max":
+            continue
+        x, _ = W.comb_batch_numpy(2, list(range(B)), N, 1.0, 5.0, max(6.0, N / 40), 0.10)
+        d_x = torch.from_numpy(x).cuda()
+        full = ext.harmonic_sum_all(x, Hmax, variant, window)
+        plan = hs.hs_plan_create_ex(N, B, Hmax, variant, "reduced", "all", window)
+        for thr in (3.0, 8.0, 40.0):
+            m = full["max"]
+            b, n = np.nonzero(m > thr)
+            ref = {"spectrum": b.astype(np.int64), "bin": n.astype(np.int64), "margin": np.abs(m - thr), "max": m,
+                   "argmax_all": full["argmax"], "second": full["second"], "gap": full["gap"]}
+            count, rec = plan.run_candidates(d_x, thr, capacity=B * N)
+            check_candidates(count, {k: v.cpu().numpy() for k, v in rec.items()}, ref, (B, N),
+                             f"all-H candidates {variant}/N={N}/Hmax={Hmax}/{window}/thr={thr}")
+        plan.hs_destroy()
 
 
 def test_every_integer_H_sampled_at_bench_size(hs, ext):
@@ -159,6 +187,48 @@ def test_2d_whole_batch(hs, ext, variant):
             plan.device_status()
             ref = ext.harmonic_sum_2d(x, Hmax, variant)
             compare(plan, got, ref, f"2-D {variant}/{out_mode}/N={N}/Z={Z}/Hmax={Hmax}", x)
+
+
+@pytest.mark.parametrize("variant", ["standard", "freqbin"])
+def test_2d_host_buffer_entry_and_launch_count(hs, variant):
+    """hs_execute_host on 2-D plans (the slab layout counts nz rows per entry; the standard sum at 8192 bins, Hmax 32,
+    reduced output runs eq. 1's register-blocked kernel and needs its tile counter in every lane's workspace), and
+    hs_plan_launches against the kernels a 2-D execute really enqueues (counted by the CUDA profiler)."""
+    N, B, slab = 8192, 5, 2
+    for Z in (3, 9):
+        x = W.exp_noise_torch(B, Z * N, 9, "cpu").view(B, Z, N).contiguous().pin_memory()
+        plan = hs.hs_plan_create_2d(N, Z, B, 32, variant, "reduced")
+        d_x = x.cuda()
+        _, vmax_d, amax_d = plan.run(d_x)
+        staging = torch.empty(plan.host_staging_bytes(slab), dtype=torch.uint8, device="cuda")
+        plan.set_host_staging(staging, slab)
+        h_max = torch.empty((B, Z, N), dtype=torch.float32).pin_memory()
+        h_amax = torch.empty((B, Z, N), dtype=torch.uint8).pin_memory()
+        plan.hs_execute_host(x, None, h_max, h_amax)
+        assert plan.device_status() == hs.HS_OK
+        assert torch.equal(h_max, vmax_d.cpu()) and torch.equal(h_amax, amax_d.cpu())
+        # launches: the standard sum = memset node + rb_kernel; freq-bin = hs_2d_kernel + the streaming kernel for the outer
+        # rows, which exist from Z = 3 on
+        assert plan.launches() == 2
+        vmax = torch.empty_like(vmax_d)
+        amax = torch.empty_like(amax_d)
+        torch.cuda.synchronize()
+        try:
+            from torch.profiler import ProfilerActivity, profile
+            with profile(activities=[ProfilerActivity.CUDA]) as prof:
+                plan.hs_execute(d_x, None, vmax, amax)
+                torch.cuda.synchronize()
+            names = [e.name for e in prof.events()
+                     if e.name.startswith("Memset") or "hs_2d_" in e.name or "rb_kernel" in e.name]
+        except Exception:                                           # (no CUPTI on this box: the count above stands alone)
+            names = []
+        if names:
+            assert len(names) == plan.launches(), names
+        plan.hs_destroy()
+    full = hs.hs_plan_create_2d(N, 3, B, 32, variant, "full")       # full output: the general kernels for both variants
+    assert full.launches() == (2 if variant == "freqbin" else 1)
+    one = hs.hs_plan_create_2d(N, 3, B, 1, "freqbin", "full")       # a single level: nothing to stream separately
+    assert one.launches() == 1
 
 
 def test_2d_recovers_an_integer_harmonic_track_and_matches_1d_on_the_zero_drift_row(hs):

@@ -136,6 +136,53 @@ def test_reduced_output_over_all_levels_is_numpy_argmax():
     assert (z["argmax"] == 0).all()
 
 
+def numpy_second(levels_first):
+    """Runner-up level from level values h[..., L, ...] with the level axis at position 1: the largest value once the best
+    level is masked out, smallest level on ties (NumPy's argmax returns the first maximum)."""
+    h = np.moveaxis(np.asarray(levels_first, dtype=np.float64), 1, -1).copy()
+    best = h.argmax(axis=-1)
+    np.put_along_axis(h, best[..., None], -np.inf, -1)
+    return h.argmax(axis=-1), h.max(axis=-1)
+
+
+def test_second_best_level_over_all_levels_is_numpy_argmax_of_the_rest():
+    """`second` (what the near-tie rule of the parity tests accepts instead of `argmax`) and `gap`, on random data and on
+    small-integer data where several levels tie exactly."""
+    rng = np.random.default_rng(16)
+    cases = [rng.standard_normal((2, 300)).astype(np.float32), rng.integers(-1, 2, (2, 300)).astype(np.float32),
+             np.zeros((1, 64), np.float32)]
+    for x in cases:
+        for variant in VARIANTS:
+            r = ext.harmonic_sum_all(x, 48, variant)
+            second, runner = numpy_second(r["sums"])
+            np.testing.assert_array_equal(r["second"], second)
+            np.testing.assert_array_equal(r["gap"], r["max"] - runner)
+            assert (r["second"] != r["argmax"]).all()
+    one = ext.harmonic_sum_all(cases[0], 1, "max")                # a single level has no runner-up
+    assert np.isinf(one["gap"]).all() and (one["second"] == 0).all()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_points_entry_matches_whole_batch_for_every_integer_H(variant):
+    """hsx_points_all (what the GPU tests sample full-size runs with) against hsx_harmonic_sum_all, which the brute-force
+    pins above fix: every level of every sampled point, Greedy's j included, both eq. 2 windows."""
+    rng = np.random.default_rng(17)
+    B, N, Hmax = 3, 500, 37
+    x = rng.standard_normal((B, N)).astype(np.float32)
+    bidx = np.concatenate([rng.integers(0, B, 200), [0, B - 1, B - 1]])
+    nidx = np.concatenate([rng.integers(0, N, 200), [0, 0, N - 1]])
+    for window in (("c2", "printed") if variant == "max" else ("c2",)):
+        whole = ext.harmonic_sum_all(x, Hmax, variant, window, want_jpath=True)
+        h, j = ext.points_all(x, Hmax, variant, bidx, nidx, window)
+        assert h.shape == (len(bidx), Hmax) and j.shape == (len(bidx), Hmax)
+        np.testing.assert_array_equal(h, whole["sums"][bidx, :, nidx])
+        np.testing.assert_array_equal(j, whole["jpath"][bidx, :, nidx])
+    with pytest.raises(ValueError):
+        ext.points_all(x, Hmax, variant, [B], [0])
+    with pytest.raises(ValueError):
+        ext.points_all(x, Hmax, variant, [0], [N])
+
+
 # ---------------------------------------------------------------------------------------------- (f)-1
 def test_power_spectrum_matches_numpy_and_is_formed_in_fp32_step_by_step():
     rng = np.random.default_rng(21)
@@ -243,6 +290,25 @@ def test_2d_integer_harmonic_track_is_fully_recovered():
         assert ext.partial_sum_2d(plane, r0, z0 + Zc, H, "freqbin") / math.sqrt(H) == pytest.approx(want, rel=1e-12)
     red = ext.harmonic_sum_2d(plane, 32, "freqbin", want_sums=False)
     assert red["argmax"][0, z0 + Zc, r0] == int(np.argmax(np.cumsum(amp.astype(np.float64))[[0, 1, 3, 7, 15, 31]] / np.sqrt([1, 2, 4, 8, 16, 32])))
+
+
+@pytest.mark.parametrize("variant", ["standard", "freqbin"])
+def test_2d_reduced_outputs_are_numpy_reductions_of_the_level_planes(variant):
+    """max / argmax / gap / second of hsx_harmonic_sum_2d on every row of the plane (not only the zero-drift one),
+    against NumPy reductions of its own level planes, which the brute-force pin above fixes; integer data for exact ties."""
+    rng = np.random.default_rng(34)
+    for plane in ((rng.standard_exponential((2, 7, 120)) - 1).astype(np.float32),
+                  rng.integers(-1, 2, (1, 5, 90)).astype(np.float32), np.zeros((1, 3, 40), np.float32)):
+        for Hmax in (32, 4):
+            r = ext.harmonic_sum_2d(plane, Hmax, variant)
+            np.testing.assert_array_equal(r["argmax"], r["sums"].argmax(axis=1))      # first maximum: smallest level (C8)
+            np.testing.assert_array_equal(r["max"], r["sums"].max(axis=1))
+            second, runner = numpy_second(r["sums"])
+            np.testing.assert_array_equal(r["second"], second)
+            np.testing.assert_array_equal(r["gap"], r["max"] - runner)
+            red = ext.harmonic_sum_2d(plane, Hmax, variant, want_sums=False)          # the reduced-only call: same values
+            for k in ("max", "argmax", "gap", "second"):
+                np.testing.assert_array_equal(red[k], r[k])
 
 
 def test_2d_constant_plane_closed_form():
