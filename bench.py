@@ -188,10 +188,84 @@ def oracle_rate(x_rows, variants, seconds, threads):
     return done / dt, dt, done
 
 
-def cpu_sample_rows(seconds, threads, nbins, variants):
+def oracle_rate_ext(wl, x, variants, seconds, threads, scale, gpu_bins_per_s):
+    """cpu_baseline of the SURVEY.md section 8(f) workloads: the extension oracle as it stands (oracle/hs_oracle_ext.c; for
+    `complex` its power spectrum followed by oracle/hs_oracle.c), one variant after the other, each for its share of
+    `seconds`, tasks spread over `threads` host threads (ctypes releases the GIL).  A task is
+        allh     512 consecutive bins at a seeded random place in one of the first 4 spectra, all 64 levels (hsx_points_all:
+                 a whole 2^18-bin spectrum of eq. 2 is minutes of work, every level being summed from scratch);
+        plane    one whole f-fdot plane, reduced output (hsx_harmonic_sum_2d);
+        complex  one whole spectrum: hsx_power_spectrum, then hso_harmonic_sum at Hmax 32, reduced output.
+    Returns (bins/s over all variants, per-variant dict, threads actually used, description of the sample, seconds)."""
+    import threading
+
+    import numpy as np
+
+    import oracle
+    from oracle import ext
+    oracle.build()
+    ext.build()
+    per, total_bins, total_dt, used = {}, 0, 0.0, 1
+    for v in variants:
+        budget = seconds / len(variants)
+        if wl == "allh":
+            rows, chunk = x[:4].cpu().numpy(), 512
+            rng = np.random.default_rng(1)
+            places = [(int(rng.integers(0, rows.shape[0])), int(rng.integers(0, rows.shape[1] - chunk))) for _ in range(1 << 16)]
+            sample = f"runs of {chunk} consecutive bins at seeded random places in the first {rows.shape[0]} spectra, 64 levels each"
+
+            def run(job, v=v, rows=rows, chunk=chunk):
+                ext.points_all(rows, 64, v, np.full(chunk, job[0]), np.arange(job[1], job[1] + chunk))
+                return chunk
+        elif wl == "plane":
+            planes = x[:min(x.shape[0], threads)].cpu().numpy()
+            places = list(range(planes.shape[0]))
+            sample = f"the first {planes.shape[0]} whole planes of {planes.shape[1]} x {planes.shape[2]} bins"
+
+            def run(job, v=v, planes=planes):
+                ext.harmonic_sum_2d(planes[job], 32, v, want_sums=False)
+                return planes[job].size
+        else:
+            F = x[:min(x.shape[0], 256)].cpu().numpy()
+            places = list(range(F.shape[0]))
+            sample = f"up to {F.shape[0]} whole spectra of {F.shape[1]} bins: power spectrum, then the harmonic sum"
+
+            def run(job, v=v, F=F):
+                oracle.harmonic_sum(ext.power_spectrum(F[job], scale), 32, v, want_sums=False, want_reduced=True)
+                return F.shape[1]
+        it, lock, done = iter(places), threading.Lock(), []
+        t0 = time.perf_counter()
+
+        def worker():
+            n = 0
+            while time.perf_counter() - t0 < budget:
+                with lock:
+                    job = next(it, None)
+                if job is None:
+                    break
+                n += run(job)
+            done.append(n)
+
+        nthreads = min(threads, len(places))
+        pool = [threading.Thread(target=worker) for _ in range(nthreads)]
+        for t in pool:
+            t.start()
+        for t in pool:
+            t.join()
+        dt = time.perf_counter() - t0
+        bins = sum(done)
+        used = max(used, nthreads)
+        per[v] = {"bins_per_s_all_threads": bins / dt, "bins_timed": bins, "seconds": dt, "threads": nthreads,
+                  "gpu_over_cpu_all_threads": (gpu_bins_per_s[v] / (bins / dt)) if v in gpu_bins_per_s and bins else None}
+        total_bins += bins
+        total_dt += dt
+    return total_bins / total_dt, per, used, sample, total_dt
+
+
+def cpu_sample_rows(seconds, threads, nbins, variants, cap=64):
     # ~0.7 s of single-thread work per 2^18-bin spectrum for the four variants together
     per_spectrum = 0.7 * (nbins / float(1 << 18)) * len(variants) / 4.0
-    return max(1, min(64, int(seconds * threads / per_spectrum)))
+    return max(1, min(cap, int(seconds * threads / per_spectrum)))
 
 
 def run_reference(args):
@@ -517,7 +591,7 @@ def main():
     cpu = None
     if rank == 0 and world == 1 and args.cpu_seconds > 0 and headline_workload:
         threads = os.cpu_count() or 1
-        crows = cpu_sample_rows(args.cpu_seconds, threads, nbins, variants)
+        crows = cpu_sample_rows(args.cpu_seconds, threads, nbins, variants, cap=256)   # (a few seconds on 16 threads)
         crows = min(crows, batch)
         x_rows = x[:crows].cpu().numpy()
         rate, dt, done = oracle_rate(x_rows, variants, args.cpu_seconds, threads)
@@ -527,13 +601,21 @@ def main():
                "flags": "gcc -std=c99 -O2 (no -ffast-math), fp64, one spectrum per task (PAPER.md:27)",
                "per_variant": oracle_per_variant(x_rows, variants, threads, {v: per_variant[v]["bins_per_s"] for v in variants}),
                "paper_context": "PAPER.md:66-71 Table 1 GPU/CPU speed-ups (hardware not stated): standard 250x, Greedy 704x, freq-bin 110x, Max 177x"}
+    elif rank == 0 and world == 1 and args.cpu_seconds > 0:
+        threads = os.cpu_count() or 1
+        rate, per_cpu, used, sample, dt = oracle_rate_ext(wl, x, variants, args.cpu_seconds, threads, scale,
+                                                          {v: per_variant[v]["bins_per_s"] for v in variants})
+        cpu = {"value": rate, "unit": "bins/s", "cores": used, "kind": "oracle", "sample": f"{sample}; {dt:.1f} s in all",
+               "gpu_over_cpu": value / rate, "cpu_model": cpu_model(),
+               "flags": "gcc -std=c99 -O2 (no -ffast-math), fp64 (the power spectrum in fp32), oracle/hs_oracle_ext.c as it stands",
+               "per_variant": per_cpu}
 
     if rank == 0:
         line = {"metric": "harmonic_sum_bins_per_s", "value": value, "unit": "bins/s", "n_gpus": world,
                 "steps": args.steps, "warmup": max(3, args.warmup), "warmup_requested": args.warmup, "ms_per_step": ms_per_step,
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": desc, "batch_per_gpu": batch, "nbins": nbins, "Hmax": Hmax, "out_mode": out_mode,
-                           "variants": variants, "algo": args.algo, "headline": not args.batch,
+                           "variants": variants, "algo": args.algo, "headline": headline_workload and not args.batch,
                            "l2": f"input {x.numel() * 4 / 2**20:.0f} MiB per variant launch vs 126 MB L2"
                                  + ("" if x.numel() * 4 > (1 << 28) else " (fits: not a headline size)"),
                            "parallelism": f"dp{world} (batch shards, no collective)",

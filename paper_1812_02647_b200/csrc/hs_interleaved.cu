@@ -431,6 +431,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
         q.freeG = -1;                                                   // (groups below R have a fresh slot: ts - R <= -1)
         q.gt = q.tt = kNoTicket;
         int pft[2] = {kNoTicket, kNoTicket};                            // the T ticket whose input is in tile b (or on its way)
+        int nft[2] = {0, 0};                                            // prefetches started into tile b (phase of tbar[b] = count - 1)
         // start the TMA copies for T ticket `t` unless it has a tile already; returns its tile, or -1 if none is free
         auto fetch = [&](int t) -> int {
             if (pft[0] == t) return 0;
@@ -439,6 +440,7 @@ il_persistent_kernel(const __grid_constant__ il_params p)
             if (bsel < 0) return -1;
             const int s = t / p.nT, idx = t - s * p.nT;
             if (!CPLX) prefetch_item(p, tiles + bsel * kTileFloats, &tbar[bsel], s, idx * kTBins);
+            nft[bsel]++;
             pft[bsel] = t;
             return bsel;
         };
@@ -480,6 +482,14 @@ il_persistent_kernel(const __grid_constant__ il_params p)
                 (void)fetch(q.tt);                                      // (a tile may have become free)
             }
             cur = nxt;
+        }
+        // Every published item has been finished by the workers, but a T ticket still in hand (a bounded wait gave up
+        // before it became runnable) may have its input on the way: the CTA must not exit with a bulk copy in flight into
+        // its shared memory, so wait for that copy to land (it always does; nobody reads it).
+        if (!CPLX) {
+#pragma unroll
+            for (int b = 0; b < 2; b++)
+                if (pft[b] != kNoTicket) hsptx::mbar_wait(&tbar[b], (uint32_t)(nft[b] - 1) & 1u);
         }
         return;
     }
