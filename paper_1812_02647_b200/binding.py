@@ -9,9 +9,12 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# HS_LIBRARY names another build of the same sources in this directory (libhs_tuning.so: the -DHS_TUNING build used by
-# the builder's sweeps and the forced-timeout test); the default is the product library.
-LIB_PATH = os.path.join(_HERE, os.path.basename(os.environ.get("HS_LIBRARY", "libhs.so")))
+# The binding reads no environment variable.  A program that wants another build of the same sources in this directory
+# (libhs_tuning.so: the -DHS_TUNING build of the builder's sweeps and of the forced-timeout test) says so in code, before
+# the first import of this module:  import paper_1812_02647_b200 as pkg; pkg.LIBRARY = "libhs_tuning.so"
+import paper_1812_02647_b200 as _pkg
+
+LIB_PATH = os.path.join(_HERE, os.path.basename(_pkg.__dict__.get("LIBRARY", "libhs.so")))
 
 HS_STANDARD, HS_MAX, HS_FREQBIN, HS_GREEDY = 0, 1, 2, 3
 HS_OUT_FULL, HS_OUT_REDUCED, HS_OUT_BOTH = 1, 2, 3

@@ -276,6 +276,47 @@ def test_scaling_shapes_short_and_long_spectra(hs, oracle, algo):
                 assert sampled_compare(hs, oracle, d_x, v, "reduced", algo, np.arange(min(B, 8)), 1500, 44, Hmax=Hmax) == 1
 
 
+@pytest.mark.parametrize("algo", FAMILIES)
+def test_scaling_sweep_every_hmax_with_slot_reuse(hs, oracle, algo):
+    """`bench.py --sweep scaling` also times Hmax 2, 8 and 16 (configs[4]).  The grouped kernel of eq. 2 keeps a different
+    set of per-harmonic arrays at Hmax 8 and 16 than at 32; 160 spectra of 2^18 bins give each of its groups several
+    spectra in a row, so every workspace slot is refilled while neighbouring groups still read theirs."""
+    N, B = 1 << 18, 160
+    d_x = W.exp_noise_torch(B, N, 8, "cuda")
+    W.inject_combs_torch(d_x, 2, 0.05, 50.0, 5000.0, 0.10)
+    ran = 0
+    for Hmax in (2, 8, 16):
+        for v in _variants_of(algo, Hmax, N):
+            ran += sampled_compare(hs, oracle, d_x, v, "reduced", algo, np.array([0, 1, 17, 18, 19, 77, 158, 159]), 1500, 66,
+                                   Hmax=Hmax, check_j=(Hmax == 16))
+    assert ran >= 3
+
+
+@pytest.mark.timeout(900, method="thread")
+def test_interleaved_kernel_soak_identical_outputs_over_many_launches(hs):
+    """The interleaved ring kernel of eq. 3 hands items between a scheduler warp and the worker warps and between CTAs
+    through counters; a hand-over bug shows up once in tens of launches (it did: 128 x 2^18 with both outputs once hung).
+    40 launches per output mode on that shape, on 2^16-bin spectra (several groups per ring step) and on 2^19-bin spectra
+    (two big slots): no wait may time out and every launch must reproduce the first one bit for bit."""
+    for B, N in ((128, 1 << 18), (512, 1 << 16), (48, 1 << 19)):
+        d_x = W.exp_noise_torch(B, N, 10, "cuda")
+        for out_mode in ("both", "reduced"):
+            plan = make_plan(hs, N, B, 32, "freqbin", out_mode, "tiled")
+            first = plan.run(d_x)
+            plan.device_status()
+            for it in range(40):
+                again = plan.run(d_x)
+                if it % 8 == 7:
+                    plan.device_status()
+                    for a, b in zip(first, again):
+                        assert (a is None and b is None) or torch.equal(a, b), f"launch {it + 2} differs ({B}x{N}, {out_mode})"
+                del again
+            plan.hs_destroy()
+            del first
+        del d_x
+        torch.cuda.empty_cache()
+
+
 @pytest.mark.parametrize("algo", [pytest.param("tiled", id="tiled"), pytest.param("direct", id="direct")])
 def test_scaling_point_with_2_to_32_input_elements(hs, oracle, algo):
     """configs[4]'s largest-offset point: 65536 spectra x 2^16 bins = 2^32 input elements (16 GiB), reduced output, as
@@ -359,7 +400,10 @@ def test_a_timed_out_wait_is_reported_by_device_status():
     build.build(tuning=True)
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     code = (
-        "import torch, paper_1812_02647_b200.binding as hs\n"
+        "import torch, paper_1812_02647_b200 as pkg\n"
+        "pkg.LIBRARY = 'libhs_tuning.so'\n"
+        "import paper_1812_02647_b200.binding as hs\n"
+        "assert hs.LIB_PATH.endswith('libhs_tuning.so')\n"
         "x = torch.randn(64, 1 << 15, device='cuda')\n"
         "bad = 0\n"
         "for v in ('max', 'freqbin', 'greedy'):\n"
@@ -372,7 +416,7 @@ def test_a_timed_out_wait_is_reported_by_device_status():
         "        assert e.code == hs.HS_ERR_DEVICE_TIMEOUT\n"
         "        bad += 1\n"
         "print('TIMEOUTS', bad)\n")
-    env = dict(os.environ, HS_LIBRARY="libhs_tuning.so", HS_SPIN_LIMIT="0", PYTHONPATH=root)
+    env = dict(os.environ, HS_SPIN_LIMIT="0", PYTHONPATH=root)        # (only the tuning build reads HS_SPIN_LIMIT)
     out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=600)
     assert out.returncode == 0, out.stderr[-2000:]
     assert int(out.stdout.split("TIMEOUTS")[1]) >= 1, out.stdout
@@ -476,6 +520,37 @@ def test_candidates_match_the_oracle(hs, oracle, variant, algo):
         plan.hs_destroy()
         ran += 1
     assert ran >= 1
+
+
+def test_candidates_at_the_bench_size(hs, oracle):
+    """hs_execute_candidates on configs[2]'s full shape (4096 x 2^18, the launch bench.py times): the count equals the
+    number of bins of the plan's own reduced maximum above the threshold (another instantiation of the same kernel: a
+    whole-batch property), and the records of a few spectra, injected ones included, are the oracle's candidates."""
+    d_x, injected = W.config2_torch("cuda")
+    B, N = d_x.shape
+    chosen = np.array(sorted(set(list(injected[:3]) + [0, 4095])))
+    x_rows = d_x[chosen].cpu().numpy()
+    for v in VARIANTS:
+        # eq. 2 sums block maxima: on noise alone its h_32 sits near 12.4 at the bins whose 32 harmonics are all in range
+        thr = 22.0 if v == "max" else 12.0
+        plan = make_plan(hs, N, B, 32, v, "reduced", "tiled")
+        _, vmax, _ = plan.run(d_x)
+        plan.device_status()
+        expected = int((vmax > thr).sum().item())
+        del vmax
+        count, rec = plan.run_candidates(d_x, thr, capacity=1 << 22)
+        plan.device_status()
+        assert count == expected and 0 < count <= (1 << 22), (v, count, expected)
+        rec = _records(rec)
+        keep = np.isin(rec["spectrum"], chosen)
+        sel = {k: a[keep] for k, a in rec.items()}
+        sel["spectrum"] = np.searchsorted(chosen, sel["spectrum"])
+        ref = oracle.candidates(x_rows, 32, v, thr)
+        check_candidates(int(keep.sum()), sel, ref, (len(chosen), N), f"{v} candidates at 4096 x 2^18")
+        assert v == "max" or len(ref["spectrum"]) > 0
+        plan.hs_destroy()
+    del d_x
+    torch.cuda.empty_cache()
 
 
 def test_candidates_capacity_count_and_errors(hs, oracle):
