@@ -20,7 +20,7 @@ _LIB = os.path.join(_HERE, "libhs_oracle_ext.so")
 
 STANDARD, MAX, FREQBIN, GREEDY = 0, 1, 2, 3
 VARIANTS = {"standard": STANDARD, "max": MAX, "freqbin": FREQBIN, "greedy": GREEDY}
-WINDOWS = {"c2": 0, "printed": 1}
+WINDOWS = {"c2": 0, "printed": 1, "interp": 2}      # "interp": eq. 1 with linearly interpolated terms (C15)
 
 _lib = None
 

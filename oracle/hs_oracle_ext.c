@@ -11,6 +11,11 @@
  *                                                                        floor((n i + H/2)/H) of CONVENTIONS.md C1
  *          eq. 2  S_H(n) = sum_{i=1..H} max_{j in W_i} xz(i n + j)       W_i = {0..i-1} (C2) or {1..i} (as printed)
  *          eq. 3, eq. 4 as in hs_oracle.c (C3, C4)
+ *        and eq. 1 with the spectrum read BETWEEN bins (reading R-INTERP, CONVENTIONS.md C15; the third sub-item of the
+ *        row).  The argument of eq. 1, n i / H, is not an integer; PAPER.md:52 is about the power a
+ *        harmonic loses when it falls between two Fourier bins.  With n i = q H + r, 0 <= r < H:
+ *          eq. 1, interpolated  S_H(n) = sum_{i=1..H} ((H - r) x(q) + r x(q + 1)) / H
+ *        the straight line through the two neighbouring bins (r = 0: the bin itself; q + 1 <= n whenever r > 0).
  *        h_H = S_H/sqrt(H); reduced output over the levels l = H - 1 = 0..Hmax-1, smallest level on ties (C8).
  * (f)-1  the step before the harmonic sum ("transformed using an FFT into frequency space. Then the
  *        harmonic sum is applied"): the normalised power spectrum of a complex Fourier series,
@@ -32,7 +37,7 @@
 #include <stdint.h>
 
 enum { HSX_STANDARD = 0, HSX_MAX = 1, HSX_FREQBIN = 2, HSX_GREEDY = 3 };
-enum { HSX_WINDOW_C2 = 0, HSX_WINDOW_PRINTED = 1 };
+enum { HSX_WINDOW_C2 = 0, HSX_WINDOW_PRINTED = 1, HSX_TERM_INTERP = 2 };   /* 2: eq. 1 only, interpolated terms */
 
 static double xz(const float *x, int64_t N, int64_t k)
 {
@@ -45,7 +50,12 @@ double hsx_partial_sum(const float *x, int64_t N, int64_t n, int H, int variant,
 {
     double S = 0.0;
     int j = 0;
-    if (variant == HSX_STANDARD) {                        /* eq. 1: x(n i / H), nearest bin, half up */
+    if (variant == HSX_STANDARD && window == HSX_TERM_INTERP) {   /* eq. 1: x(n i / H) on the line between bins */
+        for (int i = 1; i <= H; i++) {
+            const int64_t q = (n * i) / H, r = (n * i) % H;
+            S += ((double)(H - r) * (double)x[q] + (double)r * xz(x, N, q + 1)) / (double)H;
+        }
+    } else if (variant == HSX_STANDARD) {                 /* eq. 1: x(n i / H), nearest bin, half up */
         for (int i = 1; i <= H; i++)
             S += (double)x[(2 * n * i + H) / (2 * (int64_t)H)];
     } else if (variant == HSX_FREQBIN) {                  /* eq. 3 */
@@ -80,7 +90,8 @@ double hsx_partial_sum(const float *x, int64_t N, int64_t n, int H, int variant,
 int hsx_harmonic_sum_all(const float *x, int64_t N, int64_t B, int Hmax, int variant, int window,
                          double *sums, double *vmax, uint8_t *amax, double *gap, uint8_t *second, uint8_t *jpath)
 {
-    if (!x || N < 1 || B < 1 || Hmax < 1 || Hmax > 64 || variant < 0 || variant > 3 || window < 0 || window > 1) return 1;
+    if (!x || N < 1 || B < 1 || Hmax < 1 || Hmax > 64 || variant < 0 || variant > 3 || window < 0 || window > 2) return 1;
+    if (window == HSX_TERM_INTERP && variant != HSX_STANDARD) return 1;
     for (int64_t b = 0; b < B; b++) {
         const float *xb = x + b * N;
         for (int64_t n = 0; n < N; n++) {
@@ -110,6 +121,7 @@ int hsx_points_all(const float *x, int64_t N, int64_t B, int Hmax, int variant, 
                    int64_t npoints, const int64_t *bidx, const int64_t *nidx, double *h, uint8_t *j)
 {
     if (!x || N < 1 || B < 1 || Hmax < 1 || Hmax > 64 || variant < 0 || variant > 3 || npoints < 0) return 1;
+    if (window < 0 || window > 2 || (window == HSX_TERM_INTERP && variant != HSX_STANDARD)) return 1;
     for (int64_t p = 0; p < npoints; p++) {
         if (bidx[p] < 0 || bidx[p] >= B || nidx[p] < 0 || nidx[p] >= N) return 1;
         const float *xb = x + bidx[p] * N;

@@ -104,6 +104,59 @@ def test_printed_window_is_the_c2_window_of_the_spectrum_shifted_by_one_bin():
     assert a["sums"][0, 0, 7] == x[0, 8]                       # h_1(n) = x(n + 1): what the printed window implies
 
 
+# ---- eq. 1 with interpolated terms (reading R-INTERP, CONVENTIONS.md C15)
+def brute_interp(x, n, H):
+    """sum_i of the straight line through the two bins around n i / H, in exact rational arithmetic on the fp32 values."""
+    S = Fraction(0)
+    for i in range(1, H + 1):
+        p = Fraction(n * i, H)
+        q = math.floor(p)
+        w = p - q
+        right = Fraction(float(x[q + 1])) if q + 1 < len(x) else Fraction(0)
+        S += (1 - w) * Fraction(float(x[q])) + w * right
+    return S
+
+
+def test_interpolated_eq1_against_exact_rational_brute_force():
+    rng = np.random.default_rng(18)
+    x = rng.standard_normal(61).astype(np.float32)
+    ref = ext.harmonic_sum_all(x, 64, "standard", "interp")["sums"][0]
+    for H in range(1, 65):
+        for n in range(61):
+            assert ref[H - 1, n] * math.sqrt(H) == pytest.approx(float(brute_interp(x, n, H)), rel=1e-12, abs=1e-12)
+            assert ext.partial_sum(x, n, H, "standard", "interp")[0] == pytest.approx(float(brute_interp(x, n, H)), rel=1e-12, abs=1e-12)
+
+
+def test_interpolated_eq1_is_numpy_interp_and_is_exact_on_straight_lines():
+    """np.interp is the library's piecewise-linear interpolation: S_H(n) = sum_i interp(n i / H).  On a ramp x(k) = a k + b
+    the line between two bins IS the ramp, so S_H(n) = a n (H + 1)/2 + b H exactly (the nearest-bin sum is not: it rounds
+    every n i / H to a bin); h_1 = x; and at bins n that are multiples of H every harmonic sits on a bin, so the
+    interpolated and the nearest-bin sums agree there."""
+    rng = np.random.default_rng(19)
+    N = 700
+    x = rng.standard_normal(N).astype(np.float32)
+    r = ext.harmonic_sum_all(x, 64, "standard", "interp")["sums"][0]
+    nearest = ext.harmonic_sum_all(x, 64, "standard")["sums"][0]
+    n = np.arange(N, dtype=np.float64)
+    k = np.arange(N, dtype=np.float64)
+    np.testing.assert_array_equal(r[0], x)
+    for H in (2, 3, 5, 7, 16, 33, 64):
+        want = sum(np.interp(n * i / H, k, x.astype(np.float64)) for i in range(1, H + 1)) / math.sqrt(H)
+        np.testing.assert_allclose(r[H - 1], want, rtol=1e-12, atol=1e-12)
+        np.testing.assert_allclose(r[H - 1, ::H], nearest[H - 1, ::H], rtol=1e-13, atol=1e-13)
+        assert np.abs(r[H - 1] - nearest[H - 1]).max() > 0.1                       # elsewhere the two readings differ
+    ramp = (0.25 * np.arange(N) - 3.0).astype(np.float32)                          # exactly representable
+    rr = ext.harmonic_sum_all(ramp, 64, "standard", "interp")["sums"][0]
+    for H in range(1, 65):
+        np.testing.assert_allclose(rr[H - 1], (0.25 * n * (H + 1) / 2 - 3.0 * H) / math.sqrt(H), rtol=1e-13, atol=1e-12)
+    red = ext.harmonic_sum_all(x, 48, "standard", "interp")                         # reduced output: NumPy reductions
+    np.testing.assert_array_equal(red["argmax"], red["sums"].argmax(axis=1))
+    np.testing.assert_array_equal(red["max"], red["sums"].max(axis=1))
+    for bad in ("max", "freqbin", "greedy"):                                        # only eq. 1 has an argument between bins
+        with pytest.raises(ValueError):
+            ext.harmonic_sum_all(x, 8, bad, "interp")
+
+
 @pytest.mark.parametrize("variant", ["max", "freqbin", "greedy"])
 def test_partial_sums_are_cumulative_in_every_integer_H(variant):
     rng = np.random.default_rng(14)
@@ -171,7 +224,7 @@ def test_points_entry_matches_whole_batch_for_every_integer_H(variant):
     x = rng.standard_normal((B, N)).astype(np.float32)
     bidx = np.concatenate([rng.integers(0, B, 200), [0, B - 1, B - 1]])
     nidx = np.concatenate([rng.integers(0, N, 200), [0, 0, N - 1]])
-    for window in (("c2", "printed") if variant == "max" else ("c2",)):
+    for window in (("c2", "printed") if variant == "max" else ("c2", "interp") if variant == "standard" else ("c2",)):
         whole = ext.harmonic_sum_all(x, Hmax, variant, window, want_jpath=True)
         h, j = ext.points_all(x, Hmax, variant, bidx, nidx, window)
         assert h.shape == (len(bidx), Hmax) and j.shape == (len(bidx), Hmax)
