@@ -78,7 +78,10 @@ enum hs_levels {
 };
 enum hs_window {
     HS_WINDOW_C2 = 0,     /* eq. 2 window j = 0 .. i-1 (CONVENTIONS.md C2: h_1(n) = x(n))                             */
-    HS_WINDOW_PRINTED = 1 /* eq. 2 window exactly as printed, j = 1 .. i: h_1(n) = x(n + 1)             */
+    HS_WINDOW_PRINTED = 1, /* eq. 2 window exactly as printed, j = 1 .. i: h_1(n) = x(n + 1)            */
+    HS_TERM_INTERP = 2     /* eq. 1 only: the term x(n i / H) of PAPER.md:17 read on the straight line between the two
+                              neighbouring bins instead of at the nearest bin (CONVENTIONS.md C15; PAPER.md:52 is about
+                              the power lost between bins): with n i = q H + r, ((H - r) x(q) + r x(q + 1)) / H          */
 };
 
 /*
@@ -104,6 +107,8 @@ hs_plan *hs_plan_create(int64_t nbins, int64_t batch, int Hmax, int variant, int
  *            bin, half up, for any H: x(floor((2 n i + H) / (2 H))) (= CONVENTIONS.md C1 for even H); h_H = S_H / sqrt(H).
  *            nbins <= 2^24.  HS_LEVELS_DYADIC with HS_WINDOW_C2 is exactly hs_plan_create.
  *   window   HS_WINDOW_PRINTED (HS_MAX only, else HS_ERR_INVALID_ARG): eq. 2 with 1 <= j <= i as the paper prints it.
+ *            HS_TERM_INTERP (HS_STANDARD only, else HS_ERR_INVALID_ARG): eq. 1 with linearly interpolated terms, with
+ *            either choice of levels; fp32: w = fp32(r) * fp32(1/H), term = fma(w, x(q+1) - x(q), x(q)).
  * Such plans resolve to HS_ALGO_GENERAL (no workspace); hs_plan_set_algo accepts only HS_ALGO_AUTO for them.
  */
 hs_plan *hs_plan_create_ex(int64_t nbins, int64_t batch, int Hmax, int variant, int out_mode, int levels, int window);

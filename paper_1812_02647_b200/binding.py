@@ -20,9 +20,9 @@ HS_STANDARD, HS_MAX, HS_FREQBIN, HS_GREEDY = 0, 1, 2, 3
 HS_OUT_FULL, HS_OUT_REDUCED, HS_OUT_BOTH = 1, 2, 3
 HS_ALGO_AUTO, HS_ALGO_DIRECT, HS_ALGO_TILED, HS_ALGO_TWOPHASE, HS_ALGO_GATHER, HS_ALGO_GROUPED, HS_ALGO_GENERAL = 0, 1, 2, 3, 4, 5, 6
 HS_LEVELS_DYADIC, HS_LEVELS_ALL = 0, 1
-HS_WINDOW_C2, HS_WINDOW_PRINTED = 0, 1
+HS_WINDOW_C2, HS_WINDOW_PRINTED, HS_TERM_INTERP = 0, 1, 2
 LEVELS = {"dyadic": HS_LEVELS_DYADIC, "all": HS_LEVELS_ALL}
-WINDOWS = {"c2": HS_WINDOW_C2, "printed": HS_WINDOW_PRINTED}
+WINDOWS = {"c2": HS_WINDOW_C2, "printed": HS_WINDOW_PRINTED, "interp": HS_TERM_INTERP}
 (HS_OK, HS_ERR_INVALID_ARG, HS_ERR_NULL_POINTER, HS_ERR_MISALIGNED, HS_ERR_UNSUPPORTED, HS_ERR_WORKSPACE, HS_ERR_CUDA,
  HS_ERR_DEVICE_TIMEOUT) = range(8)
 HS_ERR_SCRATCH_LIMIT = 8

@@ -133,7 +133,9 @@ static hs_plan *create_plan(int64_t nbins, int64_t nz, int64_t batch, int Hmax, 
     bool bad = nbins < 4 || nbins > ((int64_t)1 << 25) || (nbins % 4) != 0 || batch < 1 || L < 1 ||
                variant < HS_STANDARD || variant > HS_GREEDY || out_mode < HS_OUT_FULL || out_mode > HS_OUT_BOTH ||
                nz < 1 || batch > ((int64_t)1 << 40) / (nbins * (nz > 0 ? nz : 1)) || batch > (int64_t)0x7fffffff;
-    bad = bad || (levels != HS_LEVELS_DYADIC && levels != HS_LEVELS_ALL) || (window != HS_WINDOW_C2 && window != HS_WINDOW_PRINTED);
+    bad = bad || (levels != HS_LEVELS_DYADIC && levels != HS_LEVELS_ALL) ||
+          (window != HS_WINDOW_C2 && window != HS_WINDOW_PRINTED && window != HS_TERM_INTERP);
+    bad = bad || (window == HS_TERM_INTERP && variant != HS_STANDARD);
     bad = bad || (all && (Hmax < 1 || Hmax > 64 || nbins > ((int64_t)1 << 24)));
     bad = bad || (window == HS_WINDOW_PRINTED && variant != HS_MAX);
     bad = bad || (nz > 1 && ((nz % 2) == 0 || nz > 4095 || all || window != HS_WINDOW_C2 ||

@@ -47,7 +47,8 @@ struct emit_any {
 };
 
 // ------------------------------------------------------------------------------------------ every integer H, 1-D
-// WINDOW: 0 = CONVENTIONS.md C2 (j = 0..i-1), 1 = as printed (j = 1..i); only eq. 2 looks at it.
+// WINDOW: 0 = CONVENTIONS.md C2 (j = 0..i-1), 1 = as printed (j = 1..i): only eq. 2 looks at these;
+//         2 = eq. 1 with interpolated terms (HS_TERM_INTERP, CONVENTIONS.md C15).
 template <int VARIANT, int OUT, int WINDOW, bool JDBG>
 __global__ void __launch_bounds__(kThreads)
 hs_allh_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__restrict__ vmax,
@@ -76,6 +77,8 @@ hs_allh_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__r
     if (live) e.level(0, S, 1.0f, plane0, N);
     if (JDBG && live) jplane0[0] = 0;
     for (int H = 2; H <= Hmax; H++) {
+        // eq. 1 sums every level from scratch: in the dyadic mode the H in between are not needed at all
+        if (VARIANT == HS_STANDARD && dyadic && (H & (H - 1)) != 0) continue;
         // eqs. 2-4, reduced output only: once harmonic H is out of range for the whole warp so is every later one and S
         // stays what it is.  h = S c_H is then monotone in H, so of the remaining levels only the first (in the dyadic mode
         // it may be the first to see the last in-range harmonics) and the last can change the maximum.
@@ -92,7 +95,26 @@ hs_allh_kernel(const float *__restrict__ x, float *__restrict__ sums, float *__r
             break;
         }
         const float cn = norm_any(H);
-        if (VARIANT == HS_STANDARD) {
+        if (VARIANT == HS_STANDARD && WINDOW == 2) {
+            // eq. 1, interpolated (C15): term i reads the line between bins q and q + 1 at n i / H = q + r / H.  (q, r) is
+            // stepped exactly from i to i + 1 by adding n = a H + c.  q + 1 <= n for every i < H (and 1 < N for n = 0), so
+            // the right neighbour is always inside the spectrum; r = 0 gives w = 0 and the term x(q) exactly.
+            const int a = nn / H, c = nn - a * H;
+            const float invH = __frcp_rn((float)H);
+            int q = 0, r = 0;
+            float T = x1;                                   // i = H: x(n)
+            for (int i = 1; i < H; i++) {
+                q += a;
+                r += c;
+                if (r >= H) {
+                    r -= H;
+                    q += 1;
+                }
+                const float x0 = __ldg(xb + q), xr = __ldg(xb + q + 1);
+                T += __fmaf_rn(__fmul_rn((float)r, invH), xr - x0, x0);
+            }
+            S = T;
+        } else if (VARIANT == HS_STANDARD) {
             // eq. 1 is not cumulative over consecutive H: every level from scratch.  Index of term i: nearest(n i / H),
             // half up = floor((2 n i + H) / (2 H)); stepped from i to i + 1 by adding 2 n = a (2 H) + c: no division per term.
             const int a = nn / H, c = 2 * (nn - a * H), d = 2 * H;
@@ -364,7 +386,9 @@ int hs_launch_general(const hs_plan *p, const hs_buffers &buf, int64_t batch, vo
         return d2_by_level<HS_FREQBIN>(p, buf, batch, stream);
     }
     switch (p->variant) {
-        case HS_STANDARD: return allh_by_out<HS_STANDARD, 0>(p, buf, batch, stream);
+        case HS_STANDARD:
+            if (p->window == HS_TERM_INTERP) return allh_by_out<HS_STANDARD, 2>(p, buf, batch, stream);
+            return allh_by_out<HS_STANDARD, 0>(p, buf, batch, stream);
         case HS_MAX:
             if (p->window == HS_WINDOW_PRINTED) return allh_by_out<HS_MAX, 1>(p, buf, batch, stream);
             return allh_by_out<HS_MAX, 0>(p, buf, batch, stream);

@@ -1,5 +1,6 @@
 """Sensitivity sweep of BASELINE.json configs[4] (Figs. 1-2): recovered signal-to-noise ratio of the four
-harmonic-sum variants for a pulsar whose frequency lies between two Fourier bins, relative to the standard sum (eq. 1).
+harmonic-sum variants (and of eq. 1 with interpolated terms) for a pulsar whose frequency lies between two Fourier bins,
+relative to the standard sum (eq. 1).
 
     python -m paper_1812_02647_b200.sensitivity [--realisations 1024] [--out gpurun_out/sensitivity.json]
 
@@ -27,7 +28,9 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-VARIANTS = ["standard", "max", "freqbin", "greedy"]
+# "standard_interp": eq. 1 with its terms read on the line between the two neighbouring bins (HS_TERM_INTERP,
+# CONVENTIONS.md C15) instead of at the nearest bin
+VARIANTS = ["standard", "max", "freqbin", "greedy", "standard_interp"]
 K0 = 1251                                   # integer part of the fundamental bin (configs[0]: 37.3 Hz -> bin 1251.58)
 DELTAS = [0.05 * k for k in range(11)]
 DUTIES = [0.01, 0.02, 0.05, 0.10, 0.20, 0.40]
@@ -76,7 +79,10 @@ def level_planes(hs, x, variant):
     """h[R][6][N] of one variant through the C ABI (hs_execute, full output, Hmax = 32)."""
     import torch
     R, N = x.shape
-    plan = hs.hs_plan_create(N, R, 32, variant, "full")
+    if variant == "standard_interp":
+        plan = hs.hs_plan_create_ex(N, R, 32, "standard", "full", "dyadic", "interp")
+    else:
+        plan = hs.hs_plan_create(N, R, 32, variant, "full")
     plan.ensure_workspace(x.device)
     sums = torch.empty((R, LEVELS, N), dtype=torch.float32, device=x.device)
     plan.hs_execute(x, sums, None, None)
@@ -92,7 +98,7 @@ def calibration(hs, x_noise):
     cal = {}
     for v in VARIANTS:
         h = level_planes(hs, x_noise, v)
-        lo, hi = (N // 32, N) if v == "standard" else (256, N // 32)
+        lo, hi = (N // 32, N) if v.startswith("standard") else (256, N // 32)
         part = h[:, :, lo:hi].double()
         cal[v] = (part.mean(dim=(0, 2)), part.std(dim=(0, 2)))
         del h, part
@@ -110,7 +116,7 @@ def recovered_snr(hs, x, cal, f_true):
         best = torch.full((x.shape[0],), -1e30, dtype=torch.float64, device=x.device)
         for l in range(LEVELS):
             H = 1 << l
-            scale = H if v == "standard" else 1
+            scale = H if v.startswith("standard") else 1
             lo = int(math.ceil(scale * (f_true - 1.0)))
             hi = int(math.floor(scale * (f_true + 1.0)))
             z = (h[:, l, lo:hi + 1].double() - mu[l]) / sd[l]

@@ -104,6 +104,72 @@ def test_eq2_window_as_printed(hs, ext):
     assert e.value.code == hs.HS_ERR_INVALID_ARG
 
 
+def test_eq1_interpolated_terms(hs, ext):
+    """HS_TERM_INTERP (CONVENTIONS.md C15): eq. 1 read on the line between the two bins around n i / H, every integer H and
+    the dyadic levels, all three output modes, whole batches against the oracle; candidates too."""
+    from parity import check_candidates
+    rng = np.random.default_rng(45)
+    for N, B, Hmax, levels in ((4, 1, 64, "all"), (100, 2, 64, "all"), (4100, 2, 64, "all"), (20000, 3, 32, "dyadic"),
+                               (1 << 15, 2, 7, "all"), (2052, 5, 1, "dyadic"), (12000, 2, 16, "dyadic")):
+        x, _ = W.comb_batch_numpy(2, list(range(B)), N, 0.5, 5.0, max(6.0, N / 40), 0.10) if N >= 256 else \
+            ((rng.standard_exponential((B, N)) - 1).astype(np.float32), None)
+        d_x = torch.from_numpy(x).cuda()
+        ref = ext.harmonic_sum_all(x, Hmax, "standard", "interp")
+        if levels == "dyadic":
+            pick = [h - 1 for h in (1, 2, 4, 8, 16, 32) if h <= Hmax]
+            ref_sums = ref["sums"][:, pick]
+            best, second, gap, m = argmax_from_levels(np.moveaxis(ref_sums, 1, -1))
+            ref = {"sums": ref_sums, "max": m, "argmax": best, "second": second, "gap": gap}
+        for out_mode in ("both", "reduced", "full"):
+            plan = hs.hs_plan_create_ex(N, B, Hmax, "standard", out_mode, levels, "interp")
+            assert plan.algo == hs.HS_ALGO_GENERAL and plan.workspace_bytes() == 0
+            assert plan.levels == (Hmax if levels == "all" else len(pick))
+            got = plan.run(d_x)
+            plan.device_status()
+            compare(plan, got, ref, f"interp eq. 1 {levels}/{out_mode}/N={N}/Hmax={Hmax}", x)
+            if out_mode == "reduced" and N >= 4100:
+                thr = 4.0
+                b, n = np.nonzero(ref["max"] > thr)
+                cref = {"spectrum": b.astype(np.int64), "bin": n.astype(np.int64), "margin": np.abs(ref["max"] - thr),
+                        "max": ref["max"], "argmax_all": ref["argmax"], "second": ref["second"], "gap": ref["gap"]}
+                count, rec = plan.run_candidates(d_x, thr, capacity=B * N)
+                check_candidates(count, {k: v.cpu().numpy() for k, v in rec.items()}, cref, (B, N), f"interp candidates N={N}")
+            plan.hs_destroy()
+    # a ramp is reproduced exactly by the line between bins: S_H(n) = a n (H + 1)/2 + b H (the nearest-bin sum is not)
+    N = 4096
+    ramp = (0.25 * np.arange(N) - 3.0).astype(np.float32)
+    plan = hs.hs_plan_create_ex(N, 1, 64, "standard", "full", "all", "interp")
+    sums, _, _ = plan.run(torch.from_numpy(ramp[None]).cuda())
+    H = np.arange(1, 65)[:, None]
+    check_sums(sums[0].cpu().numpy(), (0.25 * np.arange(N)[None, :] * (H + 1) / 2 - 3.0 * H) / np.sqrt(H), "interp ramp")
+    for variant in ("max", "freqbin", "greedy"):                        # only eq. 1 has an argument between bins
+        with pytest.raises(hs.HsError) as e:
+            hs.hs_plan_create_ex(4096, 1, 32, variant, "full", "all", "interp")
+        assert e.value.code == hs.HS_ERR_INVALID_ARG
+
+
+def test_eq1_interpolated_terms_sampled_at_bench_size(hs, ext):
+    """256 x 2^18, Hmax 64, reduced output (the shape of bench.py --workload allh), sampled outputs."""
+    B, N, Hmax = 256, 1 << 18, 64
+    d_x = W.exp_noise_torch(B, N, 7, "cuda")
+    rng = np.random.default_rng(46)
+    spectra = np.array([0, 1, 100, 255])
+    bidx = np.concatenate([rng.choice(spectra, 1200), rng.choice(spectra, 400)])
+    nidx = np.concatenate([rng.integers(0, N, 1200), rng.integers(0, 4096, 400)])
+    x_rows = d_x[spectra].cpu().numpy()
+    remap = {int(b): i for i, b in enumerate(spectra)}
+    plan = hs.hs_plan_create_ex(N, B, Hmax, "standard", "reduced", "all", "interp")
+    _, vmax, amax = plan.run(d_x)
+    plan.device_status()
+    h, _ = ext.points_all(x_rows, Hmax, "standard", np.array([remap[int(b)] for b in bidx]), nidx, "interp")
+    best, second, gap, m = argmax_from_levels(h)
+    tb, tn = torch.as_tensor(bidx, device="cuda"), torch.as_tensor(nidx, device="cuda")
+    check_sums(vmax[tb, tn].cpu().numpy(), m, "interp sampled max")
+    check_argmax(amax[tb, tn].cpu().numpy(), best, second, gap, m, "interp sampled argmax")
+    assert bool((vmax >= d_x).all())                                    # h_1 = x is one of the levels
+    plan.hs_destroy()
+
+
 def test_general_plans_reject_other_families_and_bad_arguments(hs):
     plan = hs.hs_plan_create_ex(4096, 2, 64, "freqbin", "reduced", "all", "c2")
     for algo in ("direct", "tiled", "gather"):
